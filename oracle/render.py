@@ -1,0 +1,48 @@
+"""Oracle: focus map, Eq. 7, and motion-guided depth (Fig. 1(iii), Fig. 5).
+
+  M(u,v) = (1/Z) sum_i exp( -((u-u_i)^2 + (v-v_i)^2) / (2 (sigma s_i)^2) )
+
+Brute force over every pixel and every point in fp64 (NOT the separable form a
+GPU would use).  Pixel (x, y) is centred at (u, v) = (x, y) (reading C7).
+Readings D1-D6: Z = per-frame max over the image's pixels (MAX,
+default), sum (SUM) or 1 (NONE); Z = 0 -> M = 0; guided depth G = M * D.
+Inputs are the fp32 (u_i, v_i, sigma_i) of points.py promoted exactly.
+TEST INFRASTRUCTURE ONLY.
+"""
+import numpy as np
+
+NORM_MAX, NORM_SUM, NORM_NONE = 0, 1, 2
+
+
+def unnormalised(points, width, height):
+    """U(x,y) = sum_i exp(-((x-u_i)^2+(y-v_i)^2)/(2 sigma_i^2)), fp64 [height, width]."""
+    x = np.arange(width, dtype=np.float64)[None, :]
+    y = np.arange(height, dtype=np.float64)[:, None]
+    u_map = np.zeros((height, width), dtype=np.float64)
+    for (u, v, sig) in points:
+        u, v, sig = float(u), float(v), float(sig)
+        dx = x - u
+        dy = y - v
+        u_map += np.exp(-((dx * dx) + (dy * dy)) / (2.0 * sig * sig))
+    return u_map
+
+
+def focus_map(points, width, height, norm=NORM_MAX, depth=None):
+    """Returns (M, G): fp64 [height, width]; G is None when depth is None."""
+    u_map = unnormalised(points, width, height)
+    if norm == NORM_MAX:
+        z = float(u_map.max()) if len(points) else 0.0
+    elif norm == NORM_SUM:
+        z = float(u_map.sum())
+    else:
+        z = 1.0
+    m = u_map / z if z > 0.0 else np.zeros_like(u_map)
+    g = None if depth is None else m * np.asarray(depth, dtype=np.float64)
+    return m, g
+
+
+def brute_force_pixel(points, x, y):
+    """Pure-Python single pixel of U, for the pins."""
+    import math
+    return sum(math.exp(-(((x - float(u)) ** 2) + ((y - float(v)) ** 2)) / (2.0 * float(s) * float(s)))
+               for (u, v, s) in points)

@@ -1,0 +1,132 @@
+"""Seeded synthetic inputs shaped like the paper's clips (Table 1) and
+BASELINE.json's configs.  This module serves BOTH the oracle-side tests and the
+CUDA path's tests/bench; it holds none of the method's arithmetic (no attention,
+no anchoring, no projection, no rendering) -- only random tokens, a random
+camera trajectory cut into window-local poses, and random depth.
+
+The paper's dataset and DA3's weights are not available; these inputs stand in
+for them (recipe in DESIGN.md "Input recipe").
+"""
+import math
+
+import numpy as np
+
+BASE_SEED = 260107154
+
+# BASELINE.json configs[0..4].  P = tokens/frame, N = frames in the clip.
+CONFIGS = [
+    dict(name="tiny", W=4, stride=2, N=4, P=256, H=16, D=64, layers=1,
+         width=224, height=224, fx=200.0, fy=200.0, cx=112.0, cy=112.0, fps=30,
+         step=0.1, step_sd=0.02, rot_sd=0.05, head_yaw_sd=0.0, sigma=20.0),
+    dict(name="suburban", W=8, stride=4, N=240, P=777, H=16, D=64, layers=24,
+         width=960, height=544, fx=700.0, fy=700.0, cx=480.0, cy=272.0, fps=30,
+         step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.05, sigma=20.0),
+    dict(name="city", W=16, stride=8, N=600, P=777, H=16, D=64, layers=24,
+         width=1920, height=1080, fx=1400.0, fy=1400.0, cx=960.0, cy=540.0, fps=30,
+         step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.15, sigma=20.0),
+    dict(name="campus", W=32, stride=16, N=1800, P=777, H=16, D=64, layers=24,
+         width=1920, height=1080, fx=1400.0, fy=1400.0, cx=960.0, cy=540.0, fps=60,
+         step=0.08, step_sd=0.01, rot_sd=0.1, head_yaw_sd=0.0, sigma=20.0),
+    dict(name="town", W=64, stride=32, N=720, P=777, H=16, D=64, layers=24,
+         width=3840, height=2160, fx=2800.0, fy=2800.0, cx=1920.0, cy=1080.0, fps=30,
+         step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.05, sigma=20.0),
+]
+
+
+def seed_for(config_index, stream):
+    return BASE_SEED + 1000 * config_index + stream
+
+
+def num_windows(n, w, stride):
+    return -(-(n - w) // stride) + 1
+
+
+def window_starts(n, w, stride):
+    return [min(i * stride, n - w) for i in range(num_windows(n, w, stride))]
+
+
+def qkv(windows, s_len, heads, dim, seed, device="cpu", scale=1.0):
+    """Three bf16 tensors [windows, S, H, D] ~ N(0, scale^2), seeded."""
+    import torch
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    out = []
+    for _ in range(3):
+        t = torch.randn((windows, s_len, heads, dim), generator=g, device=device,
+                        dtype=torch.float32)
+        out.append((t * scale).to(torch.bfloat16))
+    return out
+
+
+def _rot(axis, a):
+    c, s = math.cos(a), math.sin(a)
+    if axis == 0:
+        return np.array([[1, 0, 0], [0, c, -s], [0, s, c]], dtype=np.float64)
+    if axis == 1:
+        return np.array([[c, 0, s], [0, 1, 0], [-s, 0, c]], dtype=np.float64)
+    return np.array([[c, -s, 0], [s, c, 0], [0, 0, 1]], dtype=np.float64)
+
+
+def trajectory(cfg, seed, num_frames=None):
+    """World->camera poses [N,4,4] fp64 of a walking / riding camera.
+
+    OpenCV axes (x right, y down, z forward).  The body heading is a random walk
+    about Y; the camera adds head yaw and pitch/roll noise; each frame advances
+    `step + N(0, step_sd)` metres along the body heading (tiny config: along the
+    camera's own z axis).
+    """
+    n = cfg["N"] if num_frames is None else num_frames
+    rng = np.random.default_rng(seed)
+    pos = np.zeros(3)
+    heading = 0.0
+    out = np.zeros((n, 4, 4), dtype=np.float64)
+    for t in range(n):
+        if cfg["name"] == "tiny":
+            ax, ay, az = rng.normal(0.0, cfg["rot_sd"], 3)
+            r_c2w = _rot(1, ay) @ _rot(0, ax) @ _rot(2, az)
+            fwd = r_c2w[:, 2]
+        else:
+            heading += rng.normal(0.0, 0.02)
+            yaw = heading + rng.normal(0.0, cfg["head_yaw_sd"]) + rng.normal(0.0, cfg["rot_sd"])
+            pitch, roll = rng.normal(0.0, cfg["rot_sd"], 2)
+            r_c2w = _rot(1, yaw) @ _rot(0, pitch) @ _rot(2, roll)
+            fwd = _rot(1, heading)[:, 2]
+        pos = pos + fwd * (cfg["step"] + rng.normal(0.0, cfg["step_sd"]))
+        out[t, :3, :3] = r_c2w.T
+        out[t, :3, 3] = -r_c2w.T @ pos
+        out[t, 3, 3] = 1.0
+    return out
+
+
+def local_windows(global_w2c, w, stride, seed=None, perturb_rot=0.0, perturb_t=0.0):
+    """Cut a trajectory into window-local poses, fp32 [Nw, W, 4, 4].
+
+    Window n's local world is its own first camera (6-DoF gauge).  Optional
+    per-frame perturbation makes overlapping estimates disagree like a real
+    model's would.
+    """
+    n = global_w2c.shape[0]
+    starts = window_starts(n, w, stride)
+    rng = np.random.default_rng(seed)
+    out = np.zeros((len(starts), w, 4, 4), dtype=np.float32)
+    for i, s0 in enumerate(starts):
+        gauge = np.linalg.inv(global_w2c[s0])
+        for k in range(w):
+            m = global_w2c[s0 + k] @ gauge
+            if perturb_rot > 0.0 or perturb_t > 0.0:
+                e = np.eye(4)
+                a = rng.normal(0.0, perturb_rot, 3)
+                e[:3, :3] = _rot(1, a[1]) @ _rot(0, a[0]) @ _rot(2, a[2])
+                e[:3, 3] = rng.normal(0.0, perturb_t, 3)
+                m = e @ m
+            out[i, k] = m.astype(np.float32)
+    return out
+
+
+def depth(frames, height, width, seed, device="cpu"):
+    """fp32 depth ~ Uniform(1, 30) m, [frames, height, width]."""
+    import torch
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    return torch.rand((frames, height, width), generator=g, device=device,
+                      dtype=torch.float32) * 29.0 + 1.0
