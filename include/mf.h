@@ -1,0 +1,159 @@
+/* mf.h -- C ABI of the B200-native (sm_100a) motion-focus hot path.
+ *
+ * Paper: "Motion Focus Recognition in Fast-Moving Egocentric Video" (arxiv 2601.07154),
+ * cited as P:NN = line NN of PAPER.md; BJ = BASELINE.json north_star.
+ *
+ * Conventions (all entry points)
+ *  - Pointers are DEVICE memory owned by the caller unless the name ends in _host.
+ *    The library never frees or retains caller memory.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued
+ *    on it and the call returns without synchronising (the *_host variants synchronise).
+ *  - Return value is an mf_status.  On any error nothing has been enqueued.
+ *    mf_last_error() returns a thread-local, human-readable message for the last failure.
+ *  - No CPU fallback: a device that is not sm_100, an unsupported shape or a misaligned
+ *    pointer is an error.  NaN/Inf in inputs are not checked (they propagate).
+ */
+#ifndef MF_H_
+#define MF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MF_OK = 0,
+    MF_ERR_INVALID_ARG = 1,   /* bad dimension / enum / NULL pointer                    */
+    MF_ERR_UNSUPPORTED = 2,   /* valid request this build cannot run (head_dim != 64...) */
+    MF_ERR_ALIGNMENT = 3,     /* pointer not 16-byte aligned, width % 4 != 0            */
+    MF_ERR_WORKSPACE = 4,     /* workspace NULL or too small                             */
+    MF_ERR_CUDA = 5           /* CUDA runtime / driver error, no sm_100 device           */
+} mf_status;
+
+const char* mf_status_string(mf_status s);
+const char* mf_last_error(void);
+int mf_version(void);         /* major*10000 + minor*100 + patch */
+
+/* ---------------------------------------------------------------------------------------------
+ * Window attention (BJ: "cross-frame global self-attention over all S=W*P patch tokens of a
+ * window, alternating with per-frame attention"; the sliding window is P:70).
+ *
+ *   out[n,i,h,:] = sum_j softmax_j( scale * q[n,i,h,:].k[n,j,h,:] ) v[n,j,h,:]
+ *
+ * GLOBAL: j over all S = W*P tokens of window n.  FRAME: j over the tokens of i's frame
+ * (token order is frame-major, s = f*P + p).  bf16 inputs, fp32 scores/softmax/accumulation,
+ * bf16 output rounded to nearest even.
+ *
+ * q,k,v,out: bf16 [windows, S, heads, head_dim] contiguous, 16-byte aligned; out must not
+ * alias q/k/v.  lse: optional fp32 [windows, heads, S] natural-log-sum-exp of the scaled
+ * scores, or NULL.  head_dim must be 64 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
+ * selects 1/sqrt(head_dim).
+ */
+typedef enum { MF_ATTN_GLOBAL = 0, MF_ATTN_FRAME = 1 } mf_attn_mode;
+
+mf_status mf_window_attention(const void* q, const void* k, const void* v, void* out, float* lse,
+                              int windows, int frames_per_window, int tokens_per_frame,
+                              int heads, int head_dim, mf_attn_mode mode, float softmax_scale,
+                              void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Sliding-window partition ("overlapping segments of size L sharing O frames", "only
+ * the newly processed, non-overlapping frames are emitted").  stride = L - O.  The last window
+ * starts at num_frames - W when (num_frames - W) % stride != 0.  Pure host arithmetic.
+ * Returns the window count, or -1 if num_frames < W, stride < 1 or stride >= W.
+ */
+int mf_num_windows(int num_frames, int W, int stride);
+int mf_window_start(int num_frames, int W, int stride, int n);   /* -1 on bad arguments */
+
+/* ---------------------------------------------------------------------------------------------
+ * Pose chaining / incremental anchoring.
+ *
+ * local_w2c : fp32 [sequences, num_windows, W, 4, 4] row-major world->camera, each window in
+ *             its own local world.  Only the top 3x4 of each matrix is read.
+ * global_w2c: fp64 [sequences, num_frames, 4, 4]; world = window 0's local frame.
+ * Window n >= 1 is aligned to window n-1 at the last frame of window n-1 (shared because
+ * overlap >= 1).  MF_ALIGN_YAW_TRANSLATION (paper): rotation about the world Y axis by
+ * the heading of the relative rotation's forward axis, plus the translation that makes the two
+ * anchor camera centres coincide; pitch/roll of each window are kept.  MF_ALIGN_RIGID: full
+ * 6-DoF alignment.  fp64 with + - * / sqrt only, no FMA contraction, fixed left-fold order:
+ * results are bit-identical to the same operations on an IEEE-754 CPU.
+ * Errors: num_windows != mf_num_windows(num_frames, W, stride) -> MF_ERR_INVALID_ARG.
+ */
+typedef enum { MF_ALIGN_YAW_TRANSLATION = 0, MF_ALIGN_RIGID = 1 } mf_align_mode;
+
+mf_status mf_chain_poses(const float* local_w2c, int sequences, int num_windows, int W, int stride,
+                         int num_frames, mf_align_mode mode, double* global_w2c, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Motion focus (Eq. 1-7) and motion-guided depth (Fig. 1(iii), Fig. 5).
+ *
+ * For every rendered frame t in [render_begin, render_end):
+ *   Eq.1  p_t = -R_t^T t_t                       Eq.3  a_w = p_i - 2 p_{i-1} + p_{i-2}
+ *   Eq.4  a_c = R a_w                            Eq.6  (u,v) = (cx + fx ax/az, cy + fy ay/az)
+ *   Eq.7  M(x,y) = (1/Z) sum_{i in trailing n_points frames} exp(-((x-u_i)^2+(y-v_i)^2)/(2 sigma_i^2))
+ *   G(x,y) = M(x,y) * depth(x,y)
+ * Pixel (x,y) is centred at (u,v) = (x,y).  A point is skipped when it needs a frame < 0,
+ * when |a_w| < 1e-12, or when |a_z| <= eps_z*|a_c|.  sigma_i = sigma*|a_w| (MF_MAG_RAW) or
+ * sigma (MF_MAG_UNIT), clamped to >= 1e-3 px.  Z = per-frame max over pixels (MF_NORM_MAX),
+ * sum (MF_NORM_SUM) or 1 (MF_NORM_NONE); Z = 0 gives M = 0.
+ * The point stage runs in fp64 (same bit-exactness rules as mf_chain_poses); (u_i,v_i,sigma_i)
+ * are rounded once to fp32 and the render runs in fp32.
+ */
+typedef struct { double fx, fy, cx, cy; } mf_intrinsics;       /* at focus-map resolution, Eq.5 */
+typedef enum { MF_VEC_ACCEL = 0 /* Eq.3 */, MF_VEC_VELOCITY = 1 /* P:125 contrast */ } mf_vec_mode;
+typedef enum { MF_MAG_RAW = 0, MF_MAG_UNIT = 1 } mf_mag_mode;
+typedef enum { MF_NORM_MAX = 0, MF_NORM_SUM = 1, MF_NORM_NONE = 2 } mf_norm_mode;
+typedef enum { MF_PTS_CURRENT_FRAME = 0 /* R = R_t */, MF_PTS_OWN_FRAME = 1 /* R = R_i */ } mf_pts_mode;
+
+typedef struct {
+    int n_points;        /* 1..32 (paper: N = 15)                           */
+    float sigma;         /* > 0                                                    */
+    int vec;             /* mf_vec_mode                                            */
+    int mag;             /* mf_mag_mode                                            */
+    int norm;            /* mf_norm_mode                                           */
+    int pts;             /* mf_pts_mode                                            */
+    double eps_z;        /* >= 0; 1e-6 recommended                                 */
+} mf_focus_params;
+
+/* Bytes of device scratch mf_motion_focus needs for `count` rendered frames. */
+size_t mf_motion_focus_workspace_size(int count, int width, int height, int n_points);
+
+/* global_w2c: fp64 [num_frames,4,4].  depth: fp32 [count,height,width] or NULL.
+ * focus_map: fp32 [count,height,width] or NULL (points only).  guided_depth: fp32 same shape
+ * or NULL (requires depth and focus_map).  focus_uv: fp32 [count,2] (u,v) of the frame's own point, NaN
+ * if invalid, or NULL.  focus_index: int32 [count], y*width+x with x=floor(u+.5), y=floor(v+.5),
+ * -1 if invalid or off-image, or NULL.  count = render_end - render_begin.
+ * width % 4 == 0 and 16-byte aligned image pointers are required (MF_ERR_ALIGNMENT).
+ */
+mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_frames,
+                          int render_begin, int render_end, int width, int height,
+                          const float* depth, const mf_focus_params* params,
+                          float* focus_map, float* guided_depth, float* focus_uv,
+                          int32_t* focus_index, void* workspace, size_t workspace_bytes,
+                          void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Host-buffer conveniences (end-to-end path): same semantics, every pointer is HOST memory
+ * (pinned memory makes the copies asynchronous).  They allocate device buffers, copy in,
+ * run the device entry point above, copy out and synchronise `stream` before returning.
+ */
+mf_status mf_window_attention_host(const void* q, const void* k, const void* v, void* out,
+                                   int windows, int frames_per_window, int tokens_per_frame,
+                                   int heads, int head_dim, mf_attn_mode mode, float softmax_scale,
+                                   void* stream);
+
+/* local_w2c fp32 [num_windows,W,4,4] (one sequence) -> chain -> focus maps of frames
+ * [render_begin, render_end).  global_w2c (fp64 [num_frames,4,4]) may be NULL. */
+mf_status mf_chain_and_focus_host(const float* local_w2c, int num_windows, int W, int stride,
+                                  int num_frames, mf_align_mode align, mf_intrinsics K,
+                                  int render_begin, int render_end, int width, int height,
+                                  const float* depth, const mf_focus_params* params,
+                                  double* global_w2c, float* focus_map, float* guided_depth,
+                                  float* focus_uv, int32_t* focus_index, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MF_H_ */

@@ -1,0 +1,209 @@
+"""Python binding of include/mf.h: argument marshalling only (ctypes).  Every step of the path
+runs in the CUDA library; torch supplies device memory and the current stream.  There is no
+fallback: a missing library or a non-sm_100 device raises."""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmf_b200.so")
+
+ATTN_GLOBAL, ATTN_FRAME = 0, 1
+ALIGN_YAW_TRANSLATION, ALIGN_RIGID = 0, 1
+VEC_ACCEL, VEC_VELOCITY = 0, 1
+MAG_RAW, MAG_UNIT = 0, 1
+NORM_MAX, NORM_SUM, NORM_NONE = 0, 1, 2
+PTS_CURRENT_FRAME, PTS_OWN_FRAME = 0, 1
+
+EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
+           "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
+           "mf_window_attention_host", "mf_chain_and_focus_host"]
+
+
+class MfError(RuntimeError):
+    pass
+
+
+class Intrinsics(ctypes.Structure):
+    _fields_ = [("fx", ctypes.c_double), ("fy", ctypes.c_double), ("cx", ctypes.c_double), ("cy", ctypes.c_double)]
+
+
+class FocusParams(ctypes.Structure):
+    _fields_ = [("n_points", ctypes.c_int), ("sigma", ctypes.c_float), ("vec", ctypes.c_int),
+                ("mag", ctypes.c_int), ("norm", ctypes.c_int), ("pts", ctypes.c_int), ("eps_z", ctypes.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libmf_b200.so (built by paper_2601_07154_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise MfError(f"{LIB_PATH} not found: run `python -m paper_2601_07154_b200.build` "
+                          "(there is no CPU or PyTorch fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cf, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_double
+        L.mf_status_string.restype = ctypes.c_char_p
+        L.mf_status_string.argtypes = [ci]
+        L.mf_last_error.restype = ctypes.c_char_p
+        L.mf_version.restype = ci
+        L.mf_num_windows.argtypes = [ci, ci, ci]
+        L.mf_window_start.argtypes = [ci, ci, ci, ci]
+        L.mf_window_attention.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, cf, vp]
+        L.mf_chain_poses.argtypes = [vp, ci, ci, ci, ci, ci, ci, vp, vp]
+        L.mf_motion_focus_workspace_size.restype = ctypes.c_size_t
+        L.mf_motion_focus_workspace_size.argtypes = [ci, ci, ci, ci]
+        L.mf_motion_focus.argtypes = [vp, Intrinsics, ci, ci, ci, ci, ci, vp, ctypes.POINTER(FocusParams),
+                                      vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
+        L.mf_window_attention_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, cf, vp]
+        L.mf_chain_and_focus_host.argtypes = [vp, ci, ci, ci, ci, ci, Intrinsics, ci, ci, ci, ci, vp,
+                                              ctypes.POINTER(FocusParams), vp, vp, vp, vp, vp, vp]
+        _lib = L
+    return _lib
+
+
+def _check(status):
+    if status != 0:
+        L = lib()
+        raise MfError(f"{L.mf_status_string(status).decode()}: {L.mf_last_error().decode()}")
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _dev(t, dtype, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise MfError(f"{name}: expected a contiguous CUDA tensor of {dtype}")
+    return t
+
+
+def num_windows(num_frames, w, stride):
+    return lib().mf_num_windows(num_frames, w, stride)
+
+
+def window_start(num_frames, w, stride, n):
+    return lib().mf_window_start(num_frames, w, stride, n)
+
+
+def window_attention(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLOBAL, softmax_scale=0.0,
+                     out=None, return_lse=False):
+    """q,k,v: bf16 CUDA [windows, S, H, D] with S = frames_per_window*tokens_per_frame."""
+    for name, t in (("q", q), ("k", k), ("v", v)):
+        _dev(t, torch.bfloat16, name)
+    if q.dim() != 4 or k.shape != q.shape or v.shape != q.shape:
+        raise MfError("q, k, v must share the shape [windows, S, H, D]")
+    windows, s_len, heads, dim = q.shape
+    if s_len != frames_per_window * tokens_per_frame:
+        raise MfError("S != frames_per_window * tokens_per_frame")
+    if out is None:
+        out = torch.empty_like(q)
+    _dev(out, torch.bfloat16, "out")
+    lse = torch.empty((windows, heads, s_len), device=q.device, dtype=torch.float32) if return_lse else None
+    _check(lib().mf_window_attention(_ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse), windows,
+                                     frames_per_window, tokens_per_frame, heads, dim, mode,
+                                     float(softmax_scale), _stream()))
+    return (out, lse) if return_lse else out
+
+
+def chain_poses(local_w2c, stride, num_frames, mode=ALIGN_YAW_TRANSLATION):
+    """local_w2c: fp32 CUDA [sequences, num_windows, W, 4, 4] (or 4-D for one sequence) -> fp64 [.., N, 4, 4]."""
+    _dev(local_w2c, torch.float32, "local_w2c")
+    squeeze = local_w2c.dim() == 4
+    x = local_w2c.unsqueeze(0) if squeeze else local_w2c
+    if x.dim() != 5 or x.shape[-2:] != (4, 4):
+        raise MfError("local_w2c must be [sequences, num_windows, W, 4, 4]")
+    seqs, nw, w = x.shape[:3]
+    out = torch.empty((seqs, num_frames, 4, 4), device=x.device, dtype=torch.float64)
+    _check(lib().mf_chain_poses(_ptr(x), seqs, nw, w, stride, num_frames, mode, _ptr(out), _stream()))
+    return out[0] if squeeze else out
+
+
+def focus_params(n_points=15, sigma=20.0, vec=VEC_ACCEL, mag=MAG_UNIT, norm=NORM_MAX, pts=PTS_CURRENT_FRAME,
+                 eps_z=1e-6):
+    return FocusParams(n_points, sigma, vec, mag, norm, pts, eps_z)
+
+
+def motion_focus(global_w2c, fx, fy, cx, cy, width, height, params=None, depth=None, render_begin=0,
+                 render_end=None, want_map=True, want_guided=None, workspace=None, out=None):
+    """global_w2c: fp64 CUDA [N,4,4].  Returns dict(focus_map, guided_depth, focus_uv, focus_index)."""
+    _dev(global_w2c, torch.float64, "global_w2c")
+    n = global_w2c.shape[0]
+    render_end = n if render_end is None else render_end
+    count = render_end - render_begin
+    params = focus_params() if params is None else params
+    dev = global_w2c.device
+    if depth is not None:
+        _dev(depth, torch.float32, "depth")
+        if tuple(depth.shape) != (count, height, width):
+            raise MfError("depth must be [count, height, width]")
+    want_guided = (depth is not None) if want_guided is None else want_guided
+    out = {} if out is None else out
+    fmap = out.get("focus_map")
+    if want_map and fmap is None:
+        fmap = torch.empty((max(count, 0), height, width), device=dev, dtype=torch.float32)
+    guided = out.get("guided_depth")
+    if want_guided and guided is None:
+        guided = torch.empty((max(count, 0), height, width), device=dev, dtype=torch.float32)
+    uv = torch.empty((max(count, 0), 2), device=dev, dtype=torch.float32)
+    idx = torch.empty((max(count, 0),), device=dev, dtype=torch.int32)
+    need = lib().mf_motion_focus_workspace_size(count, width, height, params.n_points)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty((max(need, 16),), device=dev, dtype=torch.uint8)
+    _check(lib().mf_motion_focus(_ptr(global_w2c), Intrinsics(fx, fy, cx, cy), n, render_begin, render_end,
+                                 width, height, _ptr(depth), ctypes.byref(params), _ptr(fmap), _ptr(guided),
+                                 _ptr(uv), _ptr(idx), _ptr(workspace), workspace.numel(), _stream()))
+    return {"focus_map": fmap, "guided_depth": guided, "focus_uv": uv, "focus_index": idx,
+            "workspace": workspace}
+
+
+# ---- host-buffer entry points (end-to-end path) ---------------------------------------------------
+
+def _host(t, dtype, name):
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise MfError(f"{name}: expected a contiguous CPU tensor of {dtype}")
+    return t
+
+
+def window_attention_host(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLOBAL, softmax_scale=0.0,
+                          out=None):
+    for name, t in (("q", q), ("k", k), ("v", v)):
+        _host(t, torch.bfloat16, name)
+    windows, s_len, heads, dim = q.shape
+    if out is None:
+        out = torch.empty_like(q)
+    _check(lib().mf_window_attention_host(_ptr(q), _ptr(k), _ptr(v), _ptr(out), windows, frames_per_window,
+                                          tokens_per_frame, heads, dim, mode, float(softmax_scale), _stream()))
+    return out
+
+
+def chain_and_focus_host(local_w2c, stride, num_frames, fx, fy, cx, cy, width, height, params=None, depth=None,
+                         render_begin=0, render_end=None, align=ALIGN_YAW_TRANSLATION, out=None):
+    _host(local_w2c, torch.float32, "local_w2c")
+    nw, w = local_w2c.shape[:2]
+    render_end = num_frames if render_end is None else render_end
+    count = render_end - render_begin
+    params = focus_params() if params is None else params
+    out = {} if out is None else out
+    pin = torch.cuda.is_available()
+    mk = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=pin)
+    poses = out.get("global_w2c") if "global_w2c" in out else mk((num_frames, 4, 4), torch.float64)
+    fmap = out.get("focus_map") if "focus_map" in out else mk((count, height, width), torch.float32)
+    guided = None
+    if depth is not None:
+        _host(depth, torch.float32, "depth")
+        guided = out.get("guided_depth") if "guided_depth" in out else mk((count, height, width), torch.float32)
+    uv = mk((count, 2), torch.float32)
+    idx = mk((count,), torch.int32)
+    _check(lib().mf_chain_and_focus_host(_ptr(local_w2c), nw, w, stride, num_frames, align,
+                                         Intrinsics(fx, fy, cx, cy), render_begin, render_end, width, height,
+                                         _ptr(depth), ctypes.byref(params), _ptr(poses), _ptr(fmap), _ptr(guided),
+                                         _ptr(uv), _ptr(idx), _stream()))
+    return {"global_w2c": poses, "focus_map": fmap, "guided_depth": guided, "focus_uv": uv, "focus_index": idx}

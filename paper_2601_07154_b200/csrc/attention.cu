@@ -1,0 +1,375 @@
+// mf_window_attention: flash-style bf16 self-attention for sm_100a (BJ north_star, kernels 1 and 2).
+//
+// One CTA owns 256 query rows of one (sequence, head) as two 128-row tiles.  Roles:
+//   warps 0-3  softmax warpgroup for Q tile 0 (one thread per query row, TMEM lane = row)
+//   warps 4-7  softmax warpgroup for Q tile 1
+//   warp  8    TMA producer: Q once, then K/V tiles (128 keys x 64, SWIZZLE_128B) through a ring
+//   warp  9    tcgen05.mma issuer (warps 10-11 idle; they exist so setmaxnreg can move registers)
+//              tcgen05.mma issuer (one elected thread): S = Q K^T into TMEM, O += P V with P read
+//              from TMEM; the two Q tiles are interleaved so one tile's softmax overlaps the
+//              other tile's MMAs.
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,320) O1 [320,384) P0 [384,448) P1 [448,512).
+// Online softmax in fp32 with lazy rescaling (O and l are rescaled only when the running maximum
+// grew by more than 2^8), P rounded to bf16 for the PV MMA, O normalised by 1/l in the epilogue.
+// FRAME mode is GLOBAL mode on the same bytes viewed as [windows*W, P, H, D].
+#include "common.h"
+#include "sm100_ptx.cuh"
+
+#include <cuda_bf16.h>
+
+namespace mf {
+
+constexpr int kD = 64;                 // head_dim
+constexpr int kBM = 128;               // query rows per tile (UMMA M)
+constexpr int kBN = 128;               // keys per KV tile (UMMA N of QK^T, K extent of PV)
+constexpr int kQTiles = 2;             // Q tiles per CTA
+constexpr int kStages = 4;             // K and V ring depth
+constexpr int kTileBytes = kBM * kD * 2;           // 16 KB, also the K/V tile size
+constexpr int kThreads = 384;            // 2 softmax warpgroups + 1 warpgroup holding the TMA and MMA warps
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kColS = 0, kColO = 256, kColP = 384;
+constexpr float kRescaleThreshold = 8.0f;          // log2 units
+
+struct AttnSmem {
+    alignas(1024) uint8_t q[kQTiles][kTileBytes];
+    alignas(1024) uint8_t k[kStages][kTileBytes];
+    alignas(1024) uint8_t v[kStages][kTileBytes];
+    alignas(8) uint64_t q_full;
+    uint64_t k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages];
+    uint64_t s_full[kQTiles], p_full[kQTiles], o_final[kQTiles];
+    uint32_t tmem_base;
+};
+
+struct AttnParams {
+    int seq_len;        // tokens per attention sequence (S, or P in frame mode)
+    int heads;
+    int q_blocks;       // ceil(seq_len / 256)
+    float scale_log2;   // softmax_scale * log2(e)
+    __nv_bfloat16* out;
+    float* lse;         // [sequences, heads, seq_len] or nullptr
+};
+
+constexpr uint32_t kIdescQK = ptx::idesc_bf16_f32(kBM, kBN, 0, 0);
+constexpr uint32_t kIdescPV = ptx::idesc_bf16_f32(kBM, kD, 0, 1);      // V is MN-major ([keys][d], d contiguous)
+
+// S[tile] = Q[tile] K^T : 4 MMAs of K=16 (32-byte steps inside the 128-byte swizzle atom)
+__device__ __forceinline__ void issue_qk(uint32_t tmem_s, const uint8_t* q, const uint8_t* k) {
+    const uint64_t qd = ptx::smem_desc_sw128(ptx::smem_u32(q));
+    const uint64_t kd = ptx::smem_desc_sw128(ptx::smem_u32(k));
+#pragma unroll
+    for (int i = 0; i < kD / 16; ++i) ptx::mma_ss(tmem_s, qd + 2 * i, kd + 2 * i, kIdescQK, i > 0);
+}
+// O[tile] (+)= P[tile] V : 8 MMAs of K=16 keys; P slice = 8 TMEM columns, V slice = 16 rows = 2048 B
+__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v, bool accumulate) {
+    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v));
+#pragma unroll
+    for (int i = 0; i < kBN / 16; ++i)
+        ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
+                        const __grid_constant__ CUtensorMap map_v, const AttnParams prm) {
+    extern __shared__ uint8_t smem_raw[];
+    AttnSmem& sm = *reinterpret_cast<AttnSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // work item: q block fastest so that concurrently running CTAs share one head's K/V in L2
+    const int qb = blockIdx.x % prm.q_blocks;
+    const int head = (blockIdx.x / prm.q_blocks) % prm.heads;
+    const int seq = blockIdx.x / (prm.q_blocks * prm.heads);
+    const int row0 = qb * (kQTiles * kBM);
+    const bool tile1_live = row0 + kBM < prm.seq_len;
+    const int n_kv = (prm.seq_len + kBN - 1) / kBN;
+
+    if (warp == 8 && lane == 0) {
+        ptx::prefetch_tensormap(&map_q);
+        ptx::prefetch_tensormap(&map_k);
+        ptx::prefetch_tensormap(&map_v);
+        ptx::mbar_init(&sm.q_full, 1);
+        for (int s = 0; s < kStages; ++s) {
+            ptx::mbar_init(&sm.k_full[s], 1);
+            ptx::mbar_init(&sm.k_empty[s], 1);
+            ptx::mbar_init(&sm.v_full[s], 1);
+            ptx::mbar_init(&sm.v_empty[s], 1);
+        }
+        for (int t = 0; t < kQTiles; ++t) {
+            ptx::mbar_init(&sm.s_full[t], 1);
+            ptx::mbar_init(&sm.p_full[t], kBM);
+            ptx::mbar_init(&sm.o_final[t], 1);
+        }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 9) ptx::tmem_alloc(&sm.tmem_base, kTmemCols);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+
+    // register split: 168/thread at launch -> 232 for the softmax warpgroups, 40 for the rest
+    if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp == 8) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            ptx::mbar_arrive_expect_tx(&sm.q_full, (tile1_live ? 2 : 1) * kTileBytes);
+            ptx::tma_load_4d(sm.q[0], &map_q, &sm.q_full, 0, head, row0, seq);
+            if (tile1_live) ptx::tma_load_4d(sm.q[1], &map_q, &sm.q_full, 0, head, row0 + kBM, seq);
+            for (int j = 0; j < n_kv; ++j) {
+                const int st = j % kStages;
+                const uint32_t ph = (j / kStages) & 1;
+                ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
+                ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
+                ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, head, j * kBN, seq);
+                ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
+                ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
+                ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
+            }
+        }
+    } else if (warp == 9) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            ptx::mbar_wait(&sm.q_full, 0);
+            ptx::mbar_wait(&sm.k_full[0], 0);
+            ptx::tc_fence_after();
+            issue_qk(tmem + kColS, sm.q[0], sm.k[0]);
+            ptx::mma_commit(&sm.s_full[0]);
+            if (tile1_live) {
+                issue_qk(tmem + kColS + kBN, sm.q[1], sm.k[0]);
+                ptx::mma_commit(&sm.s_full[1]);
+            }
+            ptx::mma_commit(&sm.k_empty[0]);
+            for (int j = 0; j < n_kv; ++j) {
+                const int st = j % kStages;
+                const bool more = j + 1 < n_kv;
+                const int st1 = (j + 1) % kStages;
+                ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
+                ptx::mbar_wait(&sm.p_full[0], j & 1);
+                ptx::tc_fence_after();
+                issue_pv(tmem + kColO, tmem + kColP, sm.v[st], j > 0);
+                if (more) {
+                    ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
+                    ptx::tc_fence_after();
+                    issue_qk(tmem + kColS, sm.q[0], sm.k[st1]);
+                    ptx::mma_commit(&sm.s_full[0]);
+                } else {
+                    ptx::mma_commit(&sm.o_final[0]);
+                }
+                if (tile1_live) {
+                    ptx::mbar_wait(&sm.p_full[1], j & 1);
+                    ptx::tc_fence_after();
+                    issue_pv(tmem + kColO + kD, tmem + kColP + kBN / 2, sm.v[st], j > 0);
+                    if (more) {
+                        issue_qk(tmem + kColS + kBN, sm.q[1], sm.k[st1]);
+                        ptx::mma_commit(&sm.s_full[1]);
+                    } else {
+                        ptx::mma_commit(&sm.o_final[1]);
+                    }
+                }
+                ptx::mma_commit(&sm.v_empty[st]);
+                if (more) ptx::mma_commit(&sm.k_empty[st1]);
+            }
+        }
+    }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+        // ===================== softmax warpgroups =====================
+        const int tile = warp >> 2;                       // 0 or 1
+        if (tile == 0 || tile1_live) {
+            const int row_in_tile = (warp & 3) * 32 + lane;
+            const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
+            const uint32_t t_s = tmem + lane_addr + kColS + tile * kBN;
+            const uint32_t t_o = tmem + lane_addr + kColO + tile * kD;
+            const uint32_t t_p = tmem + lane_addr + kColP + tile * (kBN / 2);
+            float m_used = -INFINITY;                     // running max in scaled log2 units
+            float l = 0.f;
+            for (int j = 0; j < n_kv; ++j) {
+                ptx::mbar_wait(&sm.s_full[tile], j & 1);
+                ptx::tc_fence_after();
+                uint32_t s[4][32];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
+                ptx::tc_wait_ld();
+                const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
+                if (valid < kBN) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            if (32 * c + i >= valid) s[c][i] = 0xff800000u;      // -inf
+                }
+                float mx = -INFINITY;
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(s[c][i]));
+                const float m_new = fmaxf(m_used, mx * prm.scale_log2);
+                const bool grow = m_new > m_used + kRescaleThreshold;            // always true at j == 0
+                if (j == 0) {
+                    m_used = m_new;
+                } else if (__any_sync(0xffffffffu, grow)) {
+                    // S(j) complete implies PV(j-1) complete (same commit), so O is quiescent here
+                    const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
+                    if (grow) m_used = m_new;
+                    l *= alpha;
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        uint32_t o[32];
+                        ptx::tmem_ld32(t_o + 32 * c, o);
+                        ptx::tc_wait_ld();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                        ptx::tmem_st32(t_o + 32 * c, o);
+                    }
+                }
+                float sum = 0.f;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float p = ptx::ex2(fmaf(__uint_as_float(s[c][i]), prm.scale_log2, -m_used));
+                        sum += p;
+                        s[c][i] = __float_as_uint(p);
+                    }
+                }
+                l += sum;
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    uint32_t pk[32];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * c][2 * i]), __uint_as_float(s[2 * c][2 * i + 1]));
+                        pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * c + 1][2 * i]), __uint_as_float(s[2 * c + 1][2 * i + 1]));
+                    }
+                    ptx::tmem_st32(t_p + 32 * c, pk);
+                }
+                ptx::tc_wait_st();
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(&sm.p_full[tile]);
+            }
+            // ---- epilogue: O / l -> bf16 -> global ----
+            ptx::mbar_wait(&sm.o_final[tile], 0);
+            ptx::tc_fence_after();
+            const int row = row0 + tile * kBM + row_in_tile;
+            const float inv_l = 1.0f / l;
+            uint32_t o[2][32];
+            ptx::tmem_ld32(t_o, o[0]);
+            ptx::tmem_ld32(t_o + 32, o[1]);
+            ptx::tc_wait_ld();
+            if (row < prm.seq_len) {
+                const size_t tok = static_cast<size_t>(seq) * prm.seq_len + row;
+                uint4* dst = reinterpret_cast<uint4*>(prm.out + (tok * prm.heads + head) * kD);
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        uint4 w;
+                        w.x = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 0]) * inv_l, __uint_as_float(o[c][8 * i + 1]) * inv_l);
+                        w.y = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 2]) * inv_l, __uint_as_float(o[c][8 * i + 3]) * inv_l);
+                        w.z = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 4]) * inv_l, __uint_as_float(o[c][8 * i + 5]) * inv_l);
+                        w.w = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 6]) * inv_l, __uint_as_float(o[c][8 * i + 7]) * inv_l);
+                        dst[4 * c + i] = w;
+                    }
+                if (prm.lse)
+                    prm.lse[(static_cast<size_t>(seq) * prm.heads + head) * prm.seq_len + row] =
+                        (m_used + log2f(l)) * 0.6931471805599453f;
+            }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 9) ptx::tmem_dealloc(tmem, kTmemCols);
+}
+
+}  // namespace mf
+
+// ------------------------------------------------------------------------------------------------
+// Host side: tensor maps + launch
+// ------------------------------------------------------------------------------------------------
+namespace mf {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// bf16 [sequences, seq_len, heads, 64] -> 4-D map (d, head, token, sequence), box = 64 x 1 x 128 x 1
+static mf_status make_map(CUtensorMap* map, const void* base, int sequences, int seq_len, int heads) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return fail(MF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+    cuuint64_t dims[4] = {static_cast<cuuint64_t>(kD), static_cast<cuuint64_t>(heads), static_cast<cuuint64_t>(seq_len),
+                          static_cast<cuuint64_t>(sequences)};
+    cuuint64_t strides[3] = {static_cast<cuuint64_t>(kD) * 2, static_cast<cuuint64_t>(heads) * kD * 2,
+                             static_cast<cuuint64_t>(seq_len) * heads * kD * 2};
+    cuuint32_t box[4] = {kD, 1, kBM, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(MF_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", static_cast<int>(r));
+    return MF_OK;
+}
+
+}  // namespace mf
+
+extern "C" mf_status mf_window_attention(const void* q, const void* k, const void* v, void* out, float* lse,
+                                         int windows, int frames_per_window, int tokens_per_frame, int heads,
+                                         int head_dim, mf_attn_mode mode, float softmax_scale, void* stream) {
+    using namespace mf;
+    if (!q || !k || !v || !out) return fail(MF_ERR_INVALID_ARG, "mf_window_attention: NULL tensor");
+    if (windows < 1 || frames_per_window < 1 || tokens_per_frame < 1 || heads < 1)
+        return fail(MF_ERR_INVALID_ARG, "mf_window_attention: non-positive dimension");
+    if (mode != MF_ATTN_GLOBAL && mode != MF_ATTN_FRAME)
+        return fail(MF_ERR_INVALID_ARG, "mf_window_attention: bad mode %d", static_cast<int>(mode));
+    if (head_dim != kD) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: head_dim=%d (only 64 is built)", head_dim);
+    if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out))
+        return fail(MF_ERR_ALIGNMENT, "mf_window_attention: q/k/v/out must be 16-byte aligned");
+    if (out == q || out == k || out == v) return fail(MF_ERR_INVALID_ARG, "mf_window_attention: out aliases an input");
+    mf_status st = require_sm100();
+    if (st != MF_OK) return st;
+
+    // FRAME mode == GLOBAL mode on [windows*W, P, H, D] (same bytes)
+    const long long sequences_ll = mode == MF_ATTN_FRAME ? static_cast<long long>(windows) * frames_per_window : windows;
+    const long long seq_len_ll = mode == MF_ATTN_FRAME ? tokens_per_frame
+                                                       : static_cast<long long>(frames_per_window) * tokens_per_frame;
+    if (seq_len_ll > (1 << 24) || sequences_ll > (1 << 24))
+        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: sequence length / count too large");
+    const int sequences = static_cast<int>(sequences_ll), seq_len = static_cast<int>(seq_len_ll);
+
+    CUtensorMap mq, mk, mv;
+    if ((st = make_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = make_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = make_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
+
+    AttnParams prm;
+    prm.seq_len = seq_len;
+    prm.heads = heads;
+    prm.q_blocks = (seq_len + kQTiles * kBM - 1) / (kQTiles * kBM);
+    const float scale = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf(static_cast<float>(head_dim));
+    prm.scale_log2 = scale * 1.4426950408889634f;
+    prm.out = static_cast<__nv_bfloat16*>(out);
+    prm.lse = lse;
+    const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
+    if (grid > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
+    const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        MF_CUDA_OK(cudaFuncSetAttribute(window_attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(mq, mk, mv,
+                                                                                                              prm);
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}

