@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path over one synthetic clip:
+for every sliding window, `layers` alternating frame/global attention layers (mf_window_attention),
+then mf_chain_poses over all windows, then mf_motion_focus (focus map + guided depth) for every frame.
+
+Default workload: BASELINE.json configs[3] (campus-shaped, W=32 stride 16, 1800 frames at 1920x1080,
+S=24864 tokens/window, 24 layers, H=16, D=64, bf16) -- the config the metric "frames/sec at W=32" is
+quoted on.  Prints ONE JSON line.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+L2_BYTES = 126 * 2 ** 20
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = campus, W=32)")
+    ap.add_argument("--windows-per-launch", type=int, default=4)
+    ap.add_argument("--focus-chunk", type=int, default=60, help="frames per mf_motion_focus call")
+    ap.add_argument("--max-windows", type=int, default=0, help="debug: truncate the clip to this many windows")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return dict(hbm=d["hbm_gbs"], tf_burst=d["bf16_tflops"], tf_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    source="measured")
+    return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """Polls nvidia-smi during the timed region (B200_PROFILING.md clocks line)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        busy = [x for x in sm if x > 0.5 * (mx[0] if mx else 1)] or sm
+        return {"sm_mhz": busy[len(busy) // 2] if busy else None, "sm_max_mhz": mx[0] if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+class Workload:
+    def __init__(self, cfg_idx, args, device):
+        import torch
+        from paper_2601_07154_b200 import api, synth
+        self.torch, self.api, self.synth = torch, api, synth
+        cfg = dict(synth.CONFIGS[cfg_idx])
+        self.cfg, self.cfg_idx, self.device = cfg, cfg_idx, device
+        self.W, self.P, self.H, self.D = cfg["W"], cfg["P"], cfg["H"], cfg["D"]
+        self.S = self.W * self.P
+        self.stride, self.layers = cfg["stride"], cfg["layers"]
+        self.N = cfg["N"]
+        self.Nw = synth.num_windows(self.N, self.W, self.stride)
+        if args.max_windows and args.max_windows < self.Nw:
+            self.Nw = args.max_windows
+            self.N = (self.Nw - 1) * self.stride + self.W
+        self.B = max(1, min(args.windows_per_launch, self.Nw))
+        self.chunk = max(1, min(args.focus_chunk, self.N))
+        self.width, self.height = cfg["width"], cfg["height"]
+        self.n_points = 15
+        # algorithmic work
+        self.flops_global = 4.0 * self.S * self.S * self.H * self.D                  # per window-layer
+        self.flops_frame = 4.0 * self.W * self.P * self.P * self.H * self.D
+        self.n_global = self.layers // 2
+        self.n_frame = self.layers - self.n_global
+        self.flops_step = self.Nw * (self.n_global * self.flops_global + self.n_frame * self.flops_frame)
+        self.focus_bytes_step = 12.0 * self.N * self.width * self.height
+
+    # ---- device-resident inputs ----
+    def setup_device(self):
+        torch, synth = self.torch, self.synth
+        dev = self.device
+        self.q, self.k, self.v = synth.qkv(self.Nw, self.S, self.H, self.D, synth.seed_for(self.cfg_idx, 0), device=dev)
+        self.o = [torch.empty((self.B, self.S, self.H, self.D), device=dev, dtype=torch.bfloat16) for _ in range(2)]
+        traj = synth.trajectory(self.cfg, synth.seed_for(self.cfg_idx, 1), self.N)
+        self.local_np = synth.local_windows(traj, self.W, self.stride, seed=synth.seed_for(self.cfg_idx, 2),
+                                            perturb_rot=1e-3, perturb_t=1e-3)
+        self.local = torch.from_numpy(self.local_np).to(dev)
+        self.depth = synth.depth(self.N, self.height, self.width, synth.seed_for(self.cfg_idx, 3), device=dev)
+        self.fmap = torch.empty_like(self.depth)
+        self.guided = torch.empty_like(self.depth)
+        self.params = self.api.focus_params(n_points=self.n_points, sigma=self.cfg["sigma"])
+        need = self.api.lib().mf_motion_focus_workspace_size(self.chunk, self.width, self.height, self.n_points)
+        self.ws = torch.empty((need,), device=dev, dtype=torch.uint8)
+        self.launches = 0
+
+    def step_device(self, ev_global=None, ev_focus=None):
+        """One full pass, everything resident in HBM.  ev_* collect (start, end) CUDA event pairs."""
+        torch, api = self.torch, self.api
+        launches = 0
+        for b0 in range(0, self.Nw, self.B):
+            b1 = min(b0 + self.B, self.Nw)
+            qb, kb, vb = self.q[b0:b1], self.k[b0:b1], self.v[b0:b1]
+            for layer in range(self.layers):
+                mode = api.ATTN_FRAME if layer % 2 == 0 else api.ATTN_GLOBAL          # reading A3
+                out = self.o[layer % 2][: b1 - b0]
+                if ev_global is not None and mode == api.ATTN_GLOBAL:
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    api.window_attention(qb, kb, vb, self.W, self.P, mode, out=out)
+                    e1.record()
+                    ev_global.append((e0, e1, b1 - b0))
+                else:
+                    api.window_attention(qb, kb, vb, self.W, self.P, mode, out=out)
+                launches += 1
+        poses = api.chain_poses(self.local, self.stride, self.N)
+        launches += 1
+        c = self.cfg
+        for f0 in range(0, self.N, self.chunk):
+            f1 = min(f0 + self.chunk, self.N)
+            if ev_focus is not None:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+            api.motion_focus(poses, c["fx"], c["fy"], c["cx"], c["cy"], self.width, self.height, self.params,
+                             depth=self.depth[f0:f1], render_begin=f0, render_end=f1, workspace=self.ws,
+                             out={"focus_map": self.fmap[f0:f1], "guided_depth": self.guided[f0:f1]})
+            if ev_focus is not None:
+                e1.record()
+                ev_focus.append((e0, e1, f1 - f0))
+            launches += 4
+        self.launches = launches
+        return poses
+
+    # ---- end-to-end through the host-buffer C ABI ----
+    def setup_host(self):
+        torch = self.torch
+        pin = lambda t: t.cpu().pin_memory()
+        self.hq, self.hk, self.hv = pin(self.q[: self.B]), pin(self.k[: self.B]), pin(self.v[: self.B])
+        self.ho = torch.empty_like(self.hq).pin_memory()
+        self.hlocal = torch.from_numpy(self.local_np).pin_memory()
+        self.hdepth = pin(self.depth[: self.chunk])
+        self.hout = {"focus_map": torch.empty_like(self.hdepth).pin_memory(),
+                     "guided_depth": torch.empty_like(self.hdepth).pin_memory(),
+                     "global_w2c": torch.empty((self.N, 4, 4), dtype=torch.float64).pin_memory()}
+        tok = self.S * self.H * self.D * 2
+        img = self.width * self.height * 4
+        self.h2d = self.Nw * 3 * tok + self.N * img + (self.N + self.chunk - 1) // self.chunk * self.hlocal.numel() * 4
+        self.d2h = self.Nw * tok + 2 * self.N * img + (self.N + self.chunk - 1) // self.chunk * (self.N * 128 + self.chunk * 12)
+
+    def step_host(self):
+        api, c = self.api, self.cfg
+        for b0 in range(0, self.Nw, self.B):
+            nb = min(self.B, self.Nw - b0)
+            api.window_attention_host(self.hq[:nb], self.hk[:nb], self.hv[:nb], self.W, self.P, api.ATTN_FRAME,
+                                      out=self.ho[:nb], num_layers=self.layers)
+        for f0 in range(0, self.N, self.chunk):
+            f1 = min(f0 + self.chunk, self.N)
+            n = f1 - f0
+            api.chain_and_focus_host(self.hlocal, self.stride, self.N, c["fx"], c["fy"], c["cx"], c["cy"], self.width,
+                                     self.height, self.params, depth=self.hdepth[:n], render_begin=f0, render_end=f1,
+                                     out={"focus_map": self.hout["focus_map"][:n], "guided_depth": self.hout["guided_depth"][:n],
+                                          "global_w2c": self.hout["global_w2c"]})
+
+
+def oracle_sample(cfg_idx, wl_dims, rows=1024):
+    """Times the oracle, as it stands, on a bounded sample of the same workload (host cores) and
+    extrapolates to the whole clip.  Returns (frames_per_s, seconds_of_sample, description, cores)."""
+    import numpy as np
+    import torch
+    from threadpoolctl import threadpool_info
+    from oracle import attention as oa
+    from oracle import chain as oc
+    from oracle import points as op
+    from oracle import render as orr
+    from paper_2601_07154_b200 import synth
+    cfg = synth.CONFIGS[cfg_idx]
+    W, P, H, D, S, Nw, N, layers = (wl_dims[k] for k in ("W", "P", "H", "D", "S", "Nw", "N", "layers"))
+    q, k, v = (t.float().numpy().astype(np.float64) for t in synth.qkv(1, S, H, D, synth.seed_for(cfg_idx, 0)))
+    rows = min(rows, S)
+    sel = np.sort(np.random.default_rng(0).choice(S, rows, replace=False))
+    t0 = time.perf_counter()
+    oa.window_attention(q, k, v, W, P, oa.GLOBAL, rows=sel)
+    t_global = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oa.window_attention(q, k, v, W, P, oa.FRAME, rows=np.arange(P))
+    t_frame = time.perf_counter() - t0
+    traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), N)
+    loc = synth.local_windows(traj, W, cfg["stride"], seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    t0 = time.perf_counter()
+    poses = oc.chain_poses(loc.tolist(), W, cfg["stride"], N)
+    frames = op.motion_points(poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"], 15, cfg["sigma"])
+    t_pose = time.perf_counter() - t0
+    depth = synth.depth(1, cfg["height"], cfg["width"], synth.seed_for(cfg_idx, 3)).numpy()[0]
+    t0 = time.perf_counter()
+    orr.focus_map(frames[min(N - 1, 20)]["points"], cfg["width"], cfg["height"], orr.NORM_MAX, depth)
+    t_render = time.perf_counter() - t0
+    n_global = layers // 2
+    n_frame = layers - n_global
+    total = Nw * (n_global * t_global * S / rows + n_frame * t_frame * W) + t_pose + N * t_render
+    cores = len(os.sched_getaffinity(0))
+    blas = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    desc = (f"global attention: {rows} sampled query rows x {H} heads of 1 window ({t_global:.2f}s); frame attention: 1 frame x "
+            f"{H} heads ({t_frame:.2f}s); pose chain + motion points: whole clip ({t_pose:.2f}s); Eq.7 render: 1 frame "
+            f"{cfg['width']}x{cfg['height']} ({t_render:.2f}s); whole-clip seconds EXTRAPOLATED = {total:.0f}")
+    return N / total, t_global + t_frame + t_pose + t_render, desc, min(cores, blas) if blas > 1 else 1
+
+
+def dims_of(cfg_idx, args):
+    from paper_2601_07154_b200 import synth
+    c = synth.CONFIGS[cfg_idx]
+    nw = synth.num_windows(c["N"], c["W"], c["stride"])
+    n = c["N"]
+    if args.max_windows and args.max_windows < nw:
+        nw = args.max_windows
+        n = (nw - 1) * c["stride"] + c["W"]
+    return dict(W=c["W"], P=c["P"], H=c["H"], D=c["D"], S=c["W"] * c["P"], Nw=nw, N=n, layers=c["layers"])
+
+
+def config_block(cfg_idx, dims, args, extra=None):
+    from paper_2601_07154_b200 import synth
+    c = synth.CONFIGS[cfg_idx]
+    d = {"workload": f"BASELINE.json configs[{cfg_idx}] {c['name']}-shaped: W={dims['W']} stride={c['stride']} over "
+                     f"{dims['N']} frames ({dims['Nw']} windows), P={dims['P']} tokens/frame, S={dims['S']}, "
+                     f"{dims['layers']} alternating frame/global layers, H={dims['H']}, D={dims['D']}, bf16; "
+                     f"focus map + guided depth at {c['width']}x{c['height']} fp32, N_points=15, sigma={c['sigma']}",
+         "windows_per_launch": args.windows_per_launch, "focus_chunk_frames": args.focus_chunk,
+         "l2": "inputs per step exceed L2 (no flush needed)"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    dims = dims_of(args.config, args)
+    vals, secs, desc, cores = [], [], "", 1
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        fps, _, desc, cores = oracle_sample(args.config, dims, rows=256)
+        if i >= args.warmup:
+            vals.append(fps)
+            secs.append(time.perf_counter() - t0)
+    value = sum(vals) / len(vals)
+    line = {"impl": "reference", "metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)",
+            "value": value, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * sum(secs) / len(secs), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_block(args.config, dims, args),
+            "cpu_baseline": {"value": value, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2601_07154_b200 import api
+    api.lib()
+    peaks = measured_peaks()
+    wl = Workload(args.config, args, dev)
+    wl.setup_device()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def reduce_max(x):
+        if world > 1:
+            t = torch.tensor([x], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return x
+
+    for _ in range(args.warmup):
+        wl.step_device()
+    sampler = ClockSampler(local_rank)
+    ev_g, ev_f = [], []
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        wl.step_device(ev_g, ev_f)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = reduce_max(e0.elapsed_time(e1))
+    ms_step = ms_total / args.steps
+    value = world * wl.N / (ms_step * 1e-3)
+
+    g_ms = sum(a.elapsed_time(b) for a, b, _ in ev_g)
+    g_windows = sum(n for _, _, n in ev_g)
+    g_launch_ms = g_ms / max(len(ev_g), 1)
+    tflops = wl.flops_global * g_windows / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
+    f_ms = sum(a.elapsed_time(b) for a, b, _ in ev_f)
+    f_frames = sum(n for _, _, n in ev_f)
+    focus_gbs = 12.0 * f_frames * wl.width * wl.height / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": "window_attention_kernel (GLOBAL mode)", "achieved": tflops,
+                "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": tflops / peaks["tf_sustained"],
+                "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['source']}); kernel timed inside a long step",
+                "frac_of_burst": tflops / peaks["tf_burst"], "frac_of_nominal_2250": tflops / 2250.0,
+                "flops_per_launch": wl.flops_global * wl.B, "ms_per_launch": g_launch_ms,
+                "share_of_step": g_ms / ms_total, "traffic": None}
+    focus = {"bound": "hbm", "kernel": "mf_motion_focus (points+tables+norm+render, 12 B/pixel algorithmic)",
+             "achieved": focus_gbs, "peak": peaks["hbm"], "unit": "GB/s", "frac": focus_gbs / peaks["hbm"],
+             "share_of_step": f_ms / ms_total}
+
+    e2e = None
+    if not args.no_e2e:
+        wl.setup_host()
+        wl.step_host()
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 2))
+        for _ in range(n_e2e):
+            wl.step_host()
+        barrier()
+        sec = reduce_max((time.perf_counter() - t0) / n_e2e)
+        e2e = {"value": world * wl.N / sec, "unit": "frames/s", "h2d_bytes_per_step": int(wl.h2d), "d2h_bytes_per_step": int(wl.d2h),
+               "steps": n_e2e, "note": "mf_window_attention_host + mf_chain_and_focus_host on pinned host buffers"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        dims = dims_of(args.config, args)
+        fps, secs, desc, cores = oracle_sample(args.config, dims)
+        cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc, "sample_seconds": secs}
+
+    if rank == 0:
+        dims = dims_of(args.config, args)
+        line = {"metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)", "value": value,
+                "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
+                "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
+                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

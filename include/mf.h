@@ -139,10 +139,13 @@ mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_fra
  * (pinned memory makes the copies asynchronous).  They allocate device buffers, copy in,
  * run the device entry point above, copy out and synchronise `stream` before returning.
  */
+/* Runs `num_layers` attention layers on the same q/k/v (layer l uses first_mode when l is even and the
+ * other mode when l is odd; outputs ping-pong between two device buffers) and returns the last
+ * layer's output.  num_layers = 1 is a single mf_window_attention call.  Copies: q,k,v in once, out once. */
 mf_status mf_window_attention_host(const void* q, const void* k, const void* v, void* out,
                                    int windows, int frames_per_window, int tokens_per_frame,
-                                   int heads, int head_dim, mf_attn_mode mode, float softmax_scale,
-                                   void* stream);
+                                   int heads, int head_dim, int num_layers, mf_attn_mode first_mode,
+                                   float softmax_scale, void* stream);
 
 /* local_w2c fp32 [num_windows,W,4,4] (one sequence) -> chain -> focus maps of frames
  * [render_begin, render_end).  global_w2c (fp64 [num_frames,4,4]) may be NULL. */

@@ -58,7 +58,7 @@ def lib():
         L.mf_motion_focus_workspace_size.argtypes = [ci, ci, ci, ci]
         L.mf_motion_focus.argtypes = [vp, Intrinsics, ci, ci, ci, ci, ci, vp, ctypes.POINTER(FocusParams),
                                       vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
-        L.mf_window_attention_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, cf, vp]
+        L.mf_window_attention_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, vp]
         L.mf_chain_and_focus_host.argtypes = [vp, ci, ci, ci, ci, ci, Intrinsics, ci, ci, ci, ci, vp,
                                               ctypes.POINTER(FocusParams), vp, vp, vp, vp, vp, vp]
         _lib = L
@@ -173,14 +173,15 @@ def _host(t, dtype, name):
 
 
 def window_attention_host(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLOBAL, softmax_scale=0.0,
-                          out=None):
+                          out=None, num_layers=1):
     for name, t in (("q", q), ("k", k), ("v", v)):
         _host(t, torch.bfloat16, name)
     windows, s_len, heads, dim = q.shape
     if out is None:
         out = torch.empty_like(q)
     _check(lib().mf_window_attention_host(_ptr(q), _ptr(k), _ptr(v), _ptr(out), windows, frames_per_window,
-                                          tokens_per_frame, heads, dim, mode, float(softmax_scale), _stream()))
+                                          tokens_per_frame, heads, dim, num_layers, mode, float(softmax_scale),
+                                          _stream()))
     return out
 
 

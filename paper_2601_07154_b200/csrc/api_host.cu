@@ -18,24 +18,33 @@ struct DeviceBuf {
 
 extern "C" mf_status mf_window_attention_host(const void* q, const void* k, const void* v, void* out, int windows,
                                               int frames_per_window, int tokens_per_frame, int heads, int head_dim,
-                                              mf_attn_mode mode, float softmax_scale, void* stream) {
+                                              int num_layers, mf_attn_mode first_mode, float softmax_scale,
+                                              void* stream) {
     if (!q || !k || !v || !out) return mf::fail(MF_ERR_INVALID_ARG, "mf_window_attention_host: NULL tensor");
-    if (windows < 1 || frames_per_window < 1 || tokens_per_frame < 1 || heads < 1 || head_dim < 1)
+    if (windows < 1 || frames_per_window < 1 || tokens_per_frame < 1 || heads < 1 || head_dim < 1 || num_layers < 1)
         return mf::fail(MF_ERR_INVALID_ARG, "mf_window_attention_host: non-positive dimension");
+    if (first_mode != MF_ATTN_GLOBAL && first_mode != MF_ATTN_FRAME)
+        return mf::fail(MF_ERR_INVALID_ARG, "mf_window_attention_host: bad mode");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t bytes = static_cast<size_t>(windows) * frames_per_window * tokens_per_frame * heads * head_dim * 2;
-    DeviceBuf dq(s), dk(s), dv(s), dout(s);
+    DeviceBuf dq(s), dk(s), dv(s), dout(s), dout2(s);
     MF_CUDA_OK(dq.alloc(bytes));
     MF_CUDA_OK(dk.alloc(bytes));
     MF_CUDA_OK(dv.alloc(bytes));
     MF_CUDA_OK(dout.alloc(bytes));
+    if (num_layers > 1) MF_CUDA_OK(dout2.alloc(bytes));
     MF_CUDA_OK(cudaMemcpyAsync(dq.p, q, bytes, cudaMemcpyHostToDevice, s));
     MF_CUDA_OK(cudaMemcpyAsync(dk.p, k, bytes, cudaMemcpyHostToDevice, s));
     MF_CUDA_OK(cudaMemcpyAsync(dv.p, v, bytes, cudaMemcpyHostToDevice, s));
-    mf_status st = mf_window_attention(dq.p, dk.p, dv.p, dout.p, nullptr, windows, frames_per_window, tokens_per_frame,
-                                       heads, head_dim, mode, softmax_scale, stream);
-    if (st != MF_OK) return st;
-    MF_CUDA_OK(cudaMemcpyAsync(out, dout.p, bytes, cudaMemcpyDeviceToHost, s));
+    void* last = dout.p;
+    for (int l = 0; l < num_layers; ++l) {
+        const mf_attn_mode m = (l % 2 == 0) ? first_mode : (first_mode == MF_ATTN_GLOBAL ? MF_ATTN_FRAME : MF_ATTN_GLOBAL);
+        last = (l % 2 == 0) ? dout.p : dout2.p;
+        mf_status st = mf_window_attention(dq.p, dk.p, dv.p, last, nullptr, windows, frames_per_window,
+                                           tokens_per_frame, heads, head_dim, m, softmax_scale, stream);
+        if (st != MF_OK) return st;
+    }
+    MF_CUDA_OK(cudaMemcpyAsync(out, last, bytes, cudaMemcpyDeviceToHost, s));
     MF_CUDA_OK(cudaStreamSynchronize(s));
     return MF_OK;
 }

@@ -46,7 +46,8 @@ struct AttnParams {
     int q_blocks;       // ceil(seq_len / 256)
     float scale_log2;   // softmax_scale * log2(e)
     __nv_bfloat16* out;
-    float* lse;         // [sequences, heads, seq_len] or nullptr
+    float* lse;         // [windows, heads, S] or nullptr
+    int lse_frames;     // sequences per window (W in frame mode, 1 in global mode)
 };
 
 constexpr uint32_t kIdescQK = ptx::idesc_bf16_f32(kBM, kBN, 0, 0);
@@ -270,9 +271,11 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         w.w = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 6]) * inv_l, __uint_as_float(o[c][8 * i + 7]) * inv_l);
                         dst[4 * c + i] = w;
                     }
-                if (prm.lse)
-                    prm.lse[(static_cast<size_t>(seq) * prm.heads + head) * prm.seq_len + row] =
-                        (m_used + log2f(l)) * 0.6931471805599453f;
+                if (prm.lse) {
+                    const int win = seq / prm.lse_frames, frame = seq - win * prm.lse_frames;
+                    prm.lse[(static_cast<size_t>(win) * prm.heads + head) * prm.lse_frames * prm.seq_len +
+                            static_cast<size_t>(frame) * prm.seq_len + row] = (m_used + log2f(l)) * 0.6931471805599453f;
+                }
             }
         }
     }
@@ -360,6 +363,7 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     prm.scale_log2 = scale * 1.4426950408889634f;
     prm.out = static_cast<__nv_bfloat16*>(out);
     prm.lse = lse;
+    prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
     if (grid > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
