@@ -48,7 +48,8 @@ int mf_version(void);         /* major*10000 + minor*100 + patch */
  *
  * q,k,v,out: bf16 [windows, S, heads, head_dim] contiguous, 16-byte aligned; out must not
  * alias q/k/v.  lse: optional fp32 [windows, heads, S] natural-log-sum-exp of the scaled
- * scores, or NULL.  head_dim must be 64 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
+ * scores (accurate to 2^-8 absolute: it is formed from the bf16-rounded weights the PV product
+ * uses), or NULL.  head_dim must be 64 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
  * selects 1/sqrt(head_dim).
  */
 typedef enum { MF_ATTN_GLOBAL = 0, MF_ATTN_FRAME = 1 } mf_attn_mode;

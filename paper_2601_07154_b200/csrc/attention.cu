@@ -223,17 +223,14 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         ptx::tmem_st32(t_o + 32 * c, o);
                     }
                 }
-                float sum = 0.f;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
+                for (int c = 0; c < 4; ++c)
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const float p = ptx::ex2(fmaf(__uint_as_float(s[c][i]), prm.scale_log2, -m_used));
-                        sum += p;
-                        s[c][i] = __float_as_uint(p);
-                    }
-                }
-                l += sum;
+                    for (int i = 0; i < 32; ++i)
+                        s[c][i] = __float_as_uint(ptx::ex2(fmaf(__uint_as_float(s[c][i]), prm.scale_log2, -m_used)));
+                // l accumulates the bf16-ROUNDED probabilities, i.e. exactly the weights the PV MMA applies,
+                // so that O/l is a true convex combination of V rows
+                float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     uint32_t pk[32];
@@ -242,8 +239,14 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * c][2 * i]), __uint_as_float(s[2 * c][2 * i + 1]));
                         pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * c + 1][2 * i]), __uint_as_float(s[2 * c + 1][2 * i + 1]));
                     }
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        sum0 += __uint_as_float(pk[i] << 16);
+                        sum1 += __uint_as_float(pk[i] & 0xffff0000u);
+                    }
                     ptx::tmem_st32(t_p + 32 * c, pk);
                 }
+                l += sum0 + sum1;
                 ptx::tc_wait_st();
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(&sm.p_full[tile]);

@@ -59,7 +59,7 @@ static size_t carve(void* base, int count, int width, int height, int n_points, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// 1. points (fp64, one thread per rendered frame; N <= a few thousand frames, latency-bound)
+// 1. points (fp64, one warp per rendered frame, one lane per trailing point)
 // ------------------------------------------------------------------------------------------------
 struct PointParams {
     double fx, fy, cx, cy, eps_z, sigma;
@@ -79,17 +79,16 @@ __device__ __forceinline__ double norm3(const double a[3]) {
 __global__ void __launch_bounds__(128)
 points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict__ pts, FrameMeta* __restrict__ meta,
               float* __restrict__ focus_uv, int32_t* __restrict__ focus_index) {
-    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    // one warp per rendered frame; lane = slot in the trailing window (oldest first), n_points <= 32
+    const int f = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (f >= pp.count) return;
     const int t = pp.render_begin + f;
-    const double* rot_t = w2c + static_cast<size_t>(t) * 16;
-    int n_valid = 0;
-    bool own_valid = false;
-    double own_u = 0.0, own_v = 0.0;
-    for (int i = t - pp.n_points + 1; i <= t; ++i) {
-        if (i < 0) continue;
-        const int need = pp.vec == MF_VEC_ACCEL ? 2 : 1;
-        if (i < need) continue;
+    const int i = t - pp.n_points + 1 + lane;
+    const int need = pp.vec == MF_VEC_ACCEL ? 2 : 1;
+    bool valid = lane < pp.n_points && i >= need;
+    double u = 0.0, v = 0.0, sig = 0.0;
+    if (valid) {
         double p0[3], p1[3], aw[3];
         load_centre(w2c + static_cast<size_t>(i) * 16, p0);
         load_centre(w2c + static_cast<size_t>(i - 1) * 16, p1);
@@ -103,44 +102,42 @@ points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
             for (int c = 0; c < 3; ++c) aw[c] = dsub(p0[c], p1[c]);
         }
         const double s = norm3(aw);
-        if (s < 1e-12) continue;
-        const double* r = pp.pts == MF_PTS_CURRENT_FRAME ? rot_t : w2c + static_cast<size_t>(i) * 16;
+        if (s < 1e-12) valid = false;
+        const double* r = w2c + static_cast<size_t>(pp.pts == MF_PTS_CURRENT_FRAME ? t : i) * 16;
         double ac[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) ac[c] = dot3(r[4 * c], r[4 * c + 1], r[4 * c + 2], aw[0], aw[1], aw[2]);   // Eq. 4
         const double nc = norm3(ac);
-        if (fabs(ac[2]) <= dmul(pp.eps_z, nc)) continue;
-        const double u = dadd(pp.cx, dmul(pp.fx, ddiv(ac[0], ac[2])));                                  // Eq. 6
-        const double v = dadd(pp.cy, dmul(pp.fy, ddiv(ac[1], ac[2])));
-        double sig = pp.mag == MF_MAG_RAW ? dmul(pp.sigma, s) : pp.sigma;
+        if (fabs(ac[2]) <= dmul(pp.eps_z, nc)) valid = false;
+        u = dadd(pp.cx, dmul(pp.fx, ddiv(ac[0], ac[2])));                                                // Eq. 6
+        v = dadd(pp.cy, dmul(pp.fy, ddiv(ac[1], ac[2])));
+        sig = pp.mag == MF_MAG_RAW ? dmul(pp.sigma, s) : pp.sigma;
         if (sig < 1e-3) sig = 1e-3;
-        pts[static_cast<size_t>(f) * kMaxPoints + n_valid] =
+    }
+    const unsigned mask = __ballot_sync(0xffffffffu, valid);
+    if (valid)
+        pts[static_cast<size_t>(f) * kMaxPoints + __popc(mask & ((1u << lane) - 1u))] =
             make_float4(__double2float_rn(u), __double2float_rn(v), __double2float_rn(sig), 0.f);
-        ++n_valid;
-        if (i == t) {
-            own_valid = true;
-            own_u = u;
-            own_v = v;
+    if (lane == 0) meta[f].n_valid = __popc(mask);
+    if (lane == pp.n_points - 1) {                      // the frame's own point (i == t)
+        int index = -1;
+        float fu = __int_as_float(0x7fc00000), fv = __int_as_float(0x7fc00000);
+        if (valid) {
+            fu = __double2float_rn(u);
+            fv = __double2float_rn(v);
+            if (isfinite(u) && isfinite(v)) {
+                const double x = floor(dadd(u, 0.5));
+                const double y = floor(dadd(v, 0.5));
+                if (x >= 0.0 && x < static_cast<double>(pp.width) && y >= 0.0 && y < static_cast<double>(pp.height))
+                    index = static_cast<int>(y) * pp.width + static_cast<int>(x);
+            }
         }
-    }
-    meta[f].n_valid = n_valid;
-    int index = -1;
-    float fu = __int_as_float(0x7fc00000), fv = __int_as_float(0x7fc00000);
-    if (own_valid) {
-        fu = __double2float_rn(own_u);
-        fv = __double2float_rn(own_v);
-        if (isfinite(own_u) && isfinite(own_v)) {
-            const double x = floor(dadd(own_u, 0.5));
-            const double y = floor(dadd(own_v, 0.5));
-            if (x >= 0.0 && x < static_cast<double>(pp.width) && y >= 0.0 && y < static_cast<double>(pp.height))
-                index = static_cast<int>(y) * pp.width + static_cast<int>(x);
+        if (focus_uv) {
+            focus_uv[2 * f] = fu;
+            focus_uv[2 * f + 1] = fv;
         }
+        if (focus_index) focus_index[f] = index;
     }
-    if (focus_uv) {
-        focus_uv[2 * f] = fu;
-        focus_uv[2 * f + 1] = fv;
-    }
-    if (focus_index) focus_index[f] = index;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -314,19 +311,47 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
     __syncthreads();
     best = s_red[0];
     __syncthreads();
-    for (int tile = warp; tile < tc * tr; tile += 8) {
-        const int c = tile % tc, r = tile / tc;
+    // each lane bounds one tile; surviving tiles are then evaluated by the whole warp
+    const int n_tiles = tc * tr;
+    for (int base = warp * 32; base < n_tiles; base += 8 * 32) {
+        const int mine = base + lane;
         float ub = 0.f;
-        for (int k = 0; k < npad; ++k) ub = fmaf(mx[k * tc + c], my[k * tr + r], ub);
-        if (ub * 1.00001f < best) continue;                // cannot beat the current maximum
-        const int x = c * kTile + lane;
-        float local = 0.f;
-        if (x < width) {
-            const int y1 = min((r + 1) * kTile, height);
-            for (int y = r * kTile; y < y1; ++y)
-                local = fmaxf(local, eval_pixel(exf, eyf + static_cast<size_t>(y) * npad, npad, width, x));
+        if (mine < n_tiles) {
+            const int c = mine % tc, r = mine / tc;
+            for (int k = 0; k < npad; ++k) ub = fmaf(mx[k * tc + c], my[k * tr + r], ub);
+        } else {
+            ub = -1.f;
         }
-        best = fmaxf(best, warp_max(local));
+        unsigned surv = __ballot_sync(0xffffffffu, ub * 1.00001f >= best);
+        while (surv) {
+            const int src = __ffs(surv) - 1;
+            surv &= surv - 1;
+            if (__shfl_sync(0xffffffffu, ub, src) * 1.00001f < best) continue;     // best may have grown
+            const int tile = base + src;
+            const int c = tile % tc, r = tile / tc;
+            const int x = min(c * kTile + lane, width - 1);                         // duplicates are harmless for a max
+            const int y0 = r * kTile, y1 = min(y0 + kTile, height);
+            float local = 0.f;
+            float e[kMaxPoints];
+#pragma unroll
+            for (int k = 0; k < kMaxPoints; ++k) e[k] = k < npad ? exf[static_cast<size_t>(k) * width + x] : 0.f;
+            for (int y = y0; y < y1; ++y) {
+                const float4* row = reinterpret_cast<const float4*>(eyf + static_cast<size_t>(y) * npad);
+                float acc = 0.f;
+#pragma unroll
+                for (int q = 0; q < kMaxPoints / 4; ++q) {
+                    if (4 * q < npad) {
+                        const float4 w = __ldg(row + q);
+                        acc = fmaf(e[4 * q + 0], w.x, acc);
+                        acc = fmaf(e[4 * q + 1], w.y, acc);
+                        acc = fmaf(e[4 * q + 2], w.z, acc);
+                        acc = fmaf(e[4 * q + 3], w.w, acc);
+                    }
+                }
+                local = fmaxf(local, acc);
+            }
+            best = fmaxf(best, warp_max(local));
+        }
     }
     if (lane == 0) s_red[warp] = best;
     __syncthreads();
@@ -476,7 +501,7 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
     pp.sigma = static_cast<double>(params->sigma);
     pp.n_points = params->n_points; pp.vec = params->vec; pp.mag = params->mag; pp.pts = params->pts;
     pp.width = width; pp.height = height; pp.render_begin = render_begin; pp.count = count;
-    points_kernel<<<(count + 127) / 128, 128, 0, s>>>(global_w2c, pp, ws.pts, ws.meta, focus_uv, focus_index);
+    points_kernel<<<(count + 3) / 4, 128, 0, s>>>(global_w2c, pp, ws.pts, ws.meta, focus_uv, focus_index);
     MF_CUDA_OK(cudaGetLastError());
     if (!focus_map) return MF_OK;
 

@@ -47,7 +47,7 @@ def _check(api, windows, w, p, heads, mode, seed, scale=1.0, rows=None, softmax_
         g = lse_gpu.cpu().numpy().astype(np.float64)
         if rows is not None:
             g = g[:, :, rows]
-        assert np.abs(g - lse_ref).max() <= 2e-3, np.abs(g - lse_ref).max()
+        assert np.abs(g - lse_ref).max() <= 4e-3, np.abs(g - lse_ref).max()   # l sums bf16-rounded weights: |d lse| <= 2^-8
     return stats
 
 
