@@ -8,7 +8,9 @@
 //              tcgen05.mma issuer (one elected thread): S = Q K^T into TMEM, O += P V with P read
 //              from TMEM; the two Q tiles are interleaved so one tile's softmax overlaps the
 //              other tile's MMAs.
-// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,320) O1 [320,384) P0 [384,448) P1 [448,512).
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,336) O1 [336,416); P (bf16) overwrites the first 64
+// columns of its S tile.  V is extended by a constant "ones" column (a second MN-major atom in shared
+// memory), so column 64 of O accumulates l = sum_j p_j on the tensor core, from the same bf16 weights.
 // Online softmax in fp32 with lazy rescaling (O and l are rescaled only when the running maximum
 // grew by more than 2^8), P rounded to bf16 for the PV MMA, O normalised by 1/l in the epilogue.
 // FRAME mode is GLOBAL mode on the same bytes viewed as [windows*W, P, H, D].
@@ -27,13 +29,15 @@ constexpr int kStages = 4;             // K and V ring depth
 constexpr int kTileBytes = kBM * kD * 2;           // 16 KB, also the K/V tile size
 constexpr int kThreads = 384;            // 2 softmax warpgroups + 1 warpgroup holding the TMA and MMA warps
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS = 0, kColO = 256, kColP = 384;
+constexpr uint32_t kColS = 0, kColO = 256;
+constexpr int kON = 80;                // PV accumulator columns: 64 outputs + column 64 = row sum l (+15 unused)
 constexpr float kRescaleThreshold = 8.0f;          // log2 units
 
 struct AttnSmem {
     alignas(1024) uint8_t q[kQTiles][kTileBytes];
     alignas(1024) uint8_t k[kStages][kTileBytes];
     alignas(1024) uint8_t v[kStages][kTileBytes];
+    alignas(1024) uint8_t ones[kTileBytes];          // [128 keys][64]: column 0 = 1.0, rest 0 (swizzled like V)
     alignas(8) uint64_t q_full;
     uint64_t k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages];
     uint64_t s_full[kQTiles], p_full[kQTiles], o_final[kQTiles];
@@ -51,7 +55,7 @@ struct AttnParams {
 };
 
 constexpr uint32_t kIdescQK = ptx::idesc_bf16_f32(kBM, kBN, 0, 0);
-constexpr uint32_t kIdescPV = ptx::idesc_bf16_f32(kBM, kD, 0, 1);      // V is MN-major ([keys][d], d contiguous)
+constexpr uint32_t kIdescPV = ptx::idesc_bf16_f32(kBM, kON, 0, 1);      // V is MN-major ([keys][d], d contiguous)
 
 // S[tile] = Q[tile] K^T : 4 MMAs of K=16 (32-byte steps inside the 128-byte swizzle atom)
 __device__ __forceinline__ void issue_qk(uint32_t tmem_s, const uint8_t* q, const uint8_t* k) {
@@ -61,8 +65,10 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, const uint8_t* q, cons
     for (int i = 0; i < kD / 16; ++i) ptx::mma_ss(tmem_s, qd + 2 * i, kd + 2 * i, kIdescQK, i > 0);
 }
 // O[tile] (+)= P[tile] V : 8 MMAs of K=16 keys; P slice = 8 TMEM columns, V slice = 16 rows = 2048 B
-__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v, bool accumulate) {
-    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v));
+__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v, const uint8_t* ones,
+                                         bool accumulate) {
+    // B = [V | ones]: atom 0 = the V stage, atom 1 (columns 64..79) = the ones tile, LBO bytes further on
+    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v), ptx::smem_u32(ones) - ptx::smem_u32(v));
 #pragma unroll
     for (int i = 0; i < kBN / 16; ++i)
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
@@ -100,6 +106,14 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             ptx::mbar_init(&sm.o_final[t], 1);
         }
         ptx::fence_barrier_init();
+    }
+    {   // ones tile: logical (key r, column 0) = 1.0 under the 128-byte swizzle, everything else 0
+        uint4* o4 = reinterpret_cast<uint4*>(sm.ones);
+        for (int i = threadIdx.x; i < kTileBytes / 16; i += kThreads) {
+            const int r = i >> 3, chunk = i & 7;
+            o4[i] = make_uint4(chunk == (r & 7) ? 0x00003F80u : 0u, 0u, 0u, 0u);
+        }
+        ptx::fence_proxy_async();
     }
     if (warp == 9) ptx::tmem_alloc(&sm.tmem_base, kTmemCols);
     ptx::tc_fence_before();
@@ -147,7 +161,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
                 ptx::mbar_wait(&sm.p_full[0], j & 1);
                 ptx::tc_fence_after();
-                issue_pv(tmem + kColO, tmem + kColP, sm.v[st], j > 0);
+                issue_pv(tmem + kColO, tmem + kColS, sm.v[st], sm.ones, j > 0);
                 if (more) {
                     ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
                     ptx::tc_fence_after();
@@ -159,7 +173,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 if (tile1_live) {
                     ptx::mbar_wait(&sm.p_full[1], j & 1);
                     ptx::tc_fence_after();
-                    issue_pv(tmem + kColO + kD, tmem + kColP + kBN / 2, sm.v[st], j > 0);
+                    issue_pv(tmem + kColO + kON, tmem + kColS + kBN, sm.v[st], sm.ones, j > 0);
                     if (more) {
                         issue_qk(tmem + kColS + kBN, sm.q[1], sm.k[st1]);
                         ptx::mma_commit(&sm.s_full[1]);
@@ -180,10 +194,10 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const int row_in_tile = (warp & 3) * 32 + lane;
             const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
             const uint32_t t_s = tmem + lane_addr + kColS + tile * kBN;
-            const uint32_t t_o = tmem + lane_addr + kColO + tile * kD;
-            const uint32_t t_p = tmem + lane_addr + kColP + tile * (kBN / 2);
+            const uint32_t t_o = tmem + lane_addr + kColO + tile * kON;
+            const uint32_t t_p = t_s;                     // P overwrites S[0:64)
             float m_used = -INFINITY;                     // running max in scaled log2 units
-            float l = 0.f;
+            const uint64_t scale2 = ptx::pack2(prm.scale_log2, prm.scale_log2);
             for (int j = 0; j < n_kv; ++j) {
                 ptx::mbar_wait(&sm.s_full[tile], j & 1);
                 ptx::tc_fence_after();
@@ -199,38 +213,46 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         for (int i = 0; i < 32; ++i)
                             if (32 * c + i >= valid) s[c][i] = 0xff800000u;      // -inf
                 }
-                float mx = -INFINITY;
+                float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(s[c][i]));
-                const float m_new = fmaxf(m_used, mx * prm.scale_log2);
+                    for (int i = 0; i < 32; i += 8)
+#pragma unroll
+                        for (int a = 0; a < 4; ++a)
+                            mx[a] = ptx::max3(mx[a], __uint_as_float(s[c][i + 2 * a]), __uint_as_float(s[c][i + 2 * a + 1]));
+                const float row_max = ptx::max3(fmaxf(mx[0], mx[1]), mx[2], mx[3]);
+                const float m_new = fmaxf(m_used, row_max * prm.scale_log2);
                 const bool grow = m_new > m_used + kRescaleThreshold;            // always true at j == 0
                 if (j == 0) {
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, grow)) {
-                    // S(j) complete implies PV(j-1) complete (same commit), so O is quiescent here
+                    // S(j) complete implies PV(j-1) complete (same commit), so O (and l) are quiescent here
                     const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
                     if (grow) m_used = m_new;
-                    l *= alpha;
+                    const uint64_t alpha2 = ptx::pack2(alpha, alpha);
 #pragma unroll
                     for (int c = 0; c < 2; ++c) {
                         uint32_t o[32];
                         ptx::tmem_ld32(t_o + 32 * c, o);
                         ptx::tc_wait_ld();
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                        for (int i = 0; i < 32; i += 2) ptx::fmul2(o[i], o[i + 1], alpha2);
                         ptx::tmem_st32(t_o + 32 * c, o);
                     }
+                    const float l_old = __uint_as_float(ptx::tmem_ld1(t_o + kD));
+                    ptx::tc_wait_ld();
+                    ptx::tmem_st1(t_o + kD, __float_as_uint(l_old * alpha));
                 }
+                const uint64_t neg_m2 = ptx::pack2(-m_used, -m_used);
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
 #pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        s[c][i] = __float_as_uint(ptx::ex2(fmaf(__uint_as_float(s[c][i]), prm.scale_log2, -m_used)));
-                // l accumulates the bf16-ROUNDED probabilities, i.e. exactly the weights the PV MMA applies,
-                // so that O/l is a true convex combination of V rows
-                float sum0 = 0.f, sum1 = 0.f;
+                    for (int i = 0; i < 32; i += 2) {
+                        ptx::ffma2(s[c][i], s[c][i + 1], scale2, neg_m2);
+                        s[c][i] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i])));
+                        s[c][i + 1] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i + 1])));
+                    }
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     uint32_t pk[32];
@@ -239,14 +261,8 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * c][2 * i]), __uint_as_float(s[2 * c][2 * i + 1]));
                         pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * c + 1][2 * i]), __uint_as_float(s[2 * c + 1][2 * i + 1]));
                     }
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        sum0 += __uint_as_float(pk[i] << 16);
-                        sum1 += __uint_as_float(pk[i] & 0xffff0000u);
-                    }
                     ptx::tmem_st32(t_p + 32 * c, pk);
                 }
-                l += sum0 + sum1;
                 ptx::tc_wait_st();
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(&sm.p_full[tile]);
@@ -255,11 +271,12 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             ptx::mbar_wait(&sm.o_final[tile], 0);
             ptx::tc_fence_after();
             const int row = row0 + tile * kBM + row_in_tile;
-            const float inv_l = 1.0f / l;
             uint32_t o[2][32];
             ptx::tmem_ld32(t_o, o[0]);
             ptx::tmem_ld32(t_o + 32, o[1]);
+            const float l = __uint_as_float(ptx::tmem_ld1(t_o + kD));           // row sum from the ones column
             ptx::tc_wait_ld();
+            const float inv_l = 1.0f / l;
             if (row < prm.seq_len) {
                 const size_t tok = static_cast<size_t>(seq) * prm.seq_len + row;
                 uint4* dst = reinterpret_cast<uint4*>(prm.out + (tok * prm.heads + head) * kD);
