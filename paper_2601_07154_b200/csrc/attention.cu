@@ -4,16 +4,21 @@
 //   warps 0-3  softmax warpgroup for Q tile 0 (one thread per query row, TMEM lane = row)
 //   warps 4-7  softmax warpgroup for Q tile 1
 //   warp  8    TMA producer: Q once, then K/V tiles (128 keys x 64, SWIZZLE_128B) through a ring
-//   warp  9    tcgen05.mma issuer (warps 10-11 idle; they exist so setmaxnreg can move registers)
-//              tcgen05.mma issuer (one elected thread): S = Q K^T into TMEM, O += P V with P read
-//              from TMEM; the two Q tiles are interleaved so one tile's softmax overlaps the
-//              other tile's MMAs.
-// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,336) O1 [336,416); P (bf16) overwrites the first 64
-// columns of its S tile.  V is extended by a constant "ones" column (a second MN-major atom in shared
-// memory), so column 64 of O accumulates l = sum_j p_j on the tensor core, from the same bf16 weights.
-// Online softmax in fp32 with lazy rescaling (O and l are rescaled only when the running maximum
-// grew by more than 2^8), P rounded to bf16 for the PV MMA, O normalised by 1/l in the epilogue.
-// FRAME mode is GLOBAL mode on the same bytes viewed as [windows*W, P, H, D].
+//   warp  9    tcgen05.mma issuer for Q tile 0 (one elected thread)
+//   warp 10    tcgen05.mma issuer for Q tile 1 (warp 11 idle; it exists so setmaxnreg can move registers)
+// TMEM (480 of 512 columns): S0 [0,128) S1 [128,256) O0 [256,336) O1 [336,416) P0 [416,448) P1 [448,480).
+// Per KV tile j and Q tile t:  S_t(j) = Q_t K(j)^T  ->  softmax warpgroup t loads S_t(j) into registers and
+// immediately hands the S columns back (s_free), so S_t(j+1) is computed while the warpgroup is still
+// exponentiating tile j;  P_t(j) (bf16) goes to its own TMEM columns in two 64-key halves and
+// O_t += P_t(j) V(j) reads it from there, half by half.  V is extended by a constant "ones" column (a second
+// MN-major atom in shared memory), so column 64 of O accumulates l = sum_j p_j on the tensor core from the
+// same bf16 weights: O/l is an exact convex combination of V rows whatever the rounding of P.
+// The softmax warps therefore never wait for the tensor core in steady state: the exponent unit (MUFU, 16/clk/SM)
+// is the binding resource at head_dim 64, and a fixed share of the exponentials is evaluated on the FMA pipe
+// instead (Cody-Waite split + cubic, relative error 7.5e-5, invisible after rounding P to bf16).
+// Online softmax in fp32 with lazy rescaling (O and l are rescaled only when the running maximum grew by more
+// than 2^8); O is normalised by 1/l in the epilogue.  FRAME mode is GLOBAL mode on the same bytes viewed as
+// [windows*W, P, H, D].
 #include "common.h"
 #include "sm100_ptx.cuh"
 
@@ -27,11 +32,16 @@ constexpr int kBN = 128;               // keys per KV tile (UMMA N of QK^T, K ex
 constexpr int kQTiles = 2;             // Q tiles per CTA
 constexpr int kStages = 4;             // K and V ring depth
 constexpr int kTileBytes = kBM * kD * 2;           // 16 KB, also the K/V tile size
-constexpr int kThreads = 384;            // 2 softmax warpgroups + 1 warpgroup holding the TMA and MMA warps
+constexpr int kThreads = 384;          // 2 softmax warpgroups + 1 warpgroup holding the TMA and MMA warps
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kColS = 0, kColO = 256;
+constexpr uint32_t kColS = 0, kColO = 256, kColP = 416;
 constexpr int kON = 80;                // PV accumulator columns: 64 outputs + column 64 = row sum l (+15 unused)
+constexpr int kPH = 32;                // TMEM columns of one P half (64 keys, bf16)
 constexpr float kRescaleThreshold = 8.0f;          // log2 units
+#ifndef MF_POLY_PAIRS
+#define MF_POLY_PAIRS 4                // of every 16 score pairs, this many are exponentiated on the FMA pipe
+#endif
+constexpr int kPolyPairs = MF_POLY_PAIRS;
 
 struct AttnSmem {
     alignas(1024) uint8_t q[kQTiles][kTileBytes];
@@ -40,8 +50,9 @@ struct AttnSmem {
     alignas(1024) uint8_t ones[kTileBytes];          // [128 keys][64]: column 0 = 1.0, rest 0 (swizzled like V)
     alignas(8) uint64_t q_full;
     uint64_t k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages];
-    uint64_t s_full[kQTiles], p_full[kQTiles], o_final[kQTiles];
+    uint64_t s_full[kQTiles], s_free[kQTiles], p_full[2][kQTiles], pv_done[2][kQTiles];   // [half][tile]
     uint32_t tmem_base;
+    uint32_t zero;     // always 0 (see the softmax loop)
 };
 
 struct AttnParams {
@@ -64,14 +75,45 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, const uint8_t* q, cons
 #pragma unroll
     for (int i = 0; i < kD / 16; ++i) ptx::mma_ss(tmem_s, qd + 2 * i, kd + 2 * i, kIdescQK, i > 0);
 }
-// O[tile] (+)= P[tile] V : 8 MMAs of K=16 keys; P slice = 8 TMEM columns, V slice = 16 rows = 2048 B
-__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v, const uint8_t* ones,
-                                         bool accumulate) {
-    // B = [V | ones]: atom 0 = the V stage, atom 1 (columns 64..79) = the ones tile, LBO bytes further on
-    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v), ptx::smem_u32(ones) - ptx::smem_u32(v));
+// O[tile] (+)= P_half[tile] V_half : 4 MMAs of K=16 keys; P slice = 8 TMEM columns, V slice = 16 rows = 2048 B
+// v_half points at the first of the 64 key rows.  B = [V | ones]: atom 0 = the V rows, atom 1 (columns 64..79) =
+// the same rows of the ones tile, LBO bytes further on.
+__device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v_half, uint32_t ones_minus_v,
+                                              bool accumulate) {
+    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v_half), ones_minus_v);
 #pragma unroll
-    for (int i = 0; i < kBN / 16; ++i)
+    for (int i = 0; i < kBN / 32; ++i)
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
+}
+
+// (2^x0, 2^x1) on the FMA pipe.  x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a cubic (minimax in
+// relative error, 7.5e-5); n is added into the exponent field.  x is clamped to >= -125 so the result stays normal.
+__device__ __forceinline__ void exp2_poly2(uint32_t& a0, uint32_t& a1) {
+    const float x0 = fmaxf(__uint_as_float(a0), -125.0f), x1 = fmaxf(__uint_as_float(a1), -125.0f);
+    const uint64_t magic = ptx::pack2(12582912.0f, 12582912.0f);          // 1.5 * 2^23: x + magic holds round(x) in its low bits
+    const uint64_t c3 = ptx::pack2(0.055171407759189606f, 0.055171407759189606f);
+    const uint64_t c2 = ptx::pack2(0.24261075258255005f, 0.24261075258255005f);
+    const uint64_t c1 = ptx::pack2(0.6932609677314758f, 0.6932609677314758f);
+    const uint64_t c0 = ptx::pack2(0.9999281167984009f, 0.9999281167984009f);
+    const uint64_t x = ptx::pack2(x0, x1);
+    uint64_t t, n, f, p;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(x), "l"(magic));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(n) : "l"(t), "l"(magic));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(f) : "l"(x), "l"(n));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(c3), "l"(f), "l"(c2));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c1));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c0));
+    uint32_t p0, p1, t0, t1;
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(p0), "=r"(p1) : "l"(p));
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(t0), "=r"(t1) : "l"(t));
+    a0 = p0 + (t0 << 23);
+    a1 = p1 + (t1 << 23);
+}
+
+__device__ __forceinline__ void fadd2_acc(uint64_t& acc, uint32_t a0, uint32_t a1) {
+    uint64_t x;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "r"(a0), "r"(a1));
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(x));
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -93,18 +135,23 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
         ptx::prefetch_tensormap(&map_q);
         ptx::prefetch_tensormap(&map_k);
         ptx::prefetch_tensormap(&map_v);
+        const uint32_t live = tile1_live ? 2 : 1;          // MMA issuers that release every K/V stage
         ptx::mbar_init(&sm.q_full, 1);
         for (int s = 0; s < kStages; ++s) {
             ptx::mbar_init(&sm.k_full[s], 1);
-            ptx::mbar_init(&sm.k_empty[s], 1);
+            ptx::mbar_init(&sm.k_empty[s], live);
             ptx::mbar_init(&sm.v_full[s], 1);
-            ptx::mbar_init(&sm.v_empty[s], 1);
+            ptx::mbar_init(&sm.v_empty[s], live);
         }
         for (int t = 0; t < kQTiles; ++t) {
             ptx::mbar_init(&sm.s_full[t], 1);
-            ptx::mbar_init(&sm.p_full[t], kBM);
-            ptx::mbar_init(&sm.o_final[t], 1);
+            ptx::mbar_init(&sm.s_free[t], 4);              // one arrival per softmax warp
+            for (int h = 0; h < 2; ++h) {
+                ptx::mbar_init(&sm.p_full[h][t], 4);
+                ptx::mbar_init(&sm.pv_done[h][t], 1);
+            }
         }
+        sm.zero = 0;
         ptx::fence_barrier_init();
     }
     {   // ones tile: logical (key r, column 0) = 1.0 under the 128-byte swizzle, everything else 0
@@ -123,69 +170,60 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 
     // register split: 168/thread at launch -> 232 for the softmax warpgroups, 40 for the rest
     if (warp >= 8) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-    if (warp == 8) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
-            ptx::mbar_arrive_expect_tx(&sm.q_full, (tile1_live ? 2 : 1) * kTileBytes);
-            ptx::tma_load_4d(sm.q[0], &map_q, &sm.q_full, 0, head, row0, seq);
-            if (tile1_live) ptx::tma_load_4d(sm.q[1], &map_q, &sm.q_full, 0, head, row0 + kBM, seq);
-            for (int j = 0; j < n_kv; ++j) {
-                const int st = j % kStages;
-                const uint32_t ph = (j / kStages) & 1;
-                ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
-                ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
-                ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, head, j * kBN, seq);
-                ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
-                ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
-                ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == 8) {
+            // ===================== TMA producer =====================
+            if (lane == 0) {
+                ptx::mbar_arrive_expect_tx(&sm.q_full, (tile1_live ? 2 : 1) * kTileBytes);
+                ptx::tma_load_4d(sm.q[0], &map_q, &sm.q_full, 0, head, row0, seq);
+                if (tile1_live) ptx::tma_load_4d(sm.q[1], &map_q, &sm.q_full, 0, head, row0 + kBM, seq);
+                for (int j = 0; j < n_kv; ++j) {
+                    const int st = j % kStages;
+                    const uint32_t ph = (j / kStages) & 1;
+                    ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
+                    ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, head, j * kBN, seq);
+                    ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
+                    ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
+                }
             }
-        }
-    } else if (warp == 9) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
-            ptx::mbar_wait(&sm.q_full, 0);
-            ptx::mbar_wait(&sm.k_full[0], 0);
-            ptx::tc_fence_after();
-            issue_qk(tmem + kColS, sm.q[0], sm.k[0]);
-            ptx::mma_commit(&sm.s_full[0]);
-            if (tile1_live) {
-                issue_qk(tmem + kColS + kBN, sm.q[1], sm.k[0]);
-                ptx::mma_commit(&sm.s_full[1]);
-            }
-            ptx::mma_commit(&sm.k_empty[0]);
-            for (int j = 0; j < n_kv; ++j) {
-                const int st = j % kStages;
-                const bool more = j + 1 < n_kv;
-                const int st1 = (j + 1) % kStages;
-                ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
-                ptx::mbar_wait(&sm.p_full[0], j & 1);
+        } else if (warp <= 10) {
+            // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================
+            const int t = warp - 9;
+            if (lane == 0 && (t == 0 || tile1_live)) {
+                const uint32_t t_s = tmem + kColS + t * kBN, t_o = tmem + kColO + t * kON, t_p = tmem + kColP + t * kPH;
+                ptx::mbar_wait(&sm.q_full, 0);
+                ptx::mbar_wait(&sm.k_full[0], 0);
                 ptx::tc_fence_after();
-                issue_pv(tmem + kColO, tmem + kColS, sm.v[st], sm.ones, j > 0);
-                if (more) {
-                    ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
-                    ptx::tc_fence_after();
-                    issue_qk(tmem + kColS, sm.q[0], sm.k[st1]);
-                    ptx::mma_commit(&sm.s_full[0]);
-                } else {
-                    ptx::mma_commit(&sm.o_final[0]);
-                }
-                if (tile1_live) {
-                    ptx::mbar_wait(&sm.p_full[1], j & 1);
-                    ptx::tc_fence_after();
-                    issue_pv(tmem + kColO + kON, tmem + kColS + kBN, sm.v[st], sm.ones, j > 0);
-                    if (more) {
-                        issue_qk(tmem + kColS + kBN, sm.q[1], sm.k[st1]);
-                        ptx::mma_commit(&sm.s_full[1]);
-                    } else {
-                        ptx::mma_commit(&sm.o_final[1]);
+                issue_qk(t_s, sm.q[t], sm.k[0]);
+                ptx::mma_commit(&sm.s_full[t]);
+                ptx::mma_commit(&sm.k_empty[0]);
+                for (int j = 0; j < n_kv; ++j) {
+                    const int st = j % kStages;
+                    if (j + 1 < n_kv) {
+                        // S(j+1) as soon as the softmax warpgroup holds S(j) in registers
+                        const int st1 = (j + 1) % kStages;
+                        ptx::mbar_wait(&sm.s_free[t], j & 1);
+                        ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
+                        ptx::tc_fence_after();
+                        issue_qk(t_s, sm.q[t], sm.k[st1]);
+                        ptx::mma_commit(&sm.s_full[t]);
+                        ptx::mma_commit(&sm.k_empty[st1]);
                     }
+                    ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
+                    const uint32_t ones_minus_v = ptx::smem_u32(sm.ones) - ptx::smem_u32(sm.v[st]);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        ptx::mbar_wait(&sm.p_full[h][t], j & 1);
+                        ptx::tc_fence_after();
+                        issue_pv_half(t_o, t_p, sm.v[st] + h * (kTileBytes / 2), ones_minus_v, j > 0 || h > 0);
+                        ptx::mma_commit(&sm.pv_done[h][t]);
+                    }
+                    ptx::mma_commit(&sm.v_empty[st]);
                 }
-                ptx::mma_commit(&sm.v_empty[st]);
-                if (more) ptx::mma_commit(&sm.k_empty[st1]);
             }
         }
-    }
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
         // ===================== softmax warpgroups =====================
@@ -195,7 +233,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
             const uint32_t t_s = tmem + lane_addr + kColS + tile * kBN;
             const uint32_t t_o = tmem + lane_addr + kColO + tile * kON;
-            const uint32_t t_p = t_s;                     // P overwrites S[0:64)
+            const uint32_t t_p = tmem + lane_addr + kColP + tile * kPH;
             float m_used = -INFINITY;                     // running max in scaled log2 units
             const uint64_t scale2 = ptx::pack2(prm.scale_log2, prm.scale_log2);
             for (int j = 0; j < n_kv; ++j) {
@@ -205,6 +243,9 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 #pragma unroll
                 for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
                 ptx::tc_wait_ld();
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by S(j+1)
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
 #pragma unroll
@@ -227,7 +268,9 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 if (j == 0) {
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, grow)) {
-                    // S(j) complete implies PV(j-1) complete (same commit), so O (and l) are quiescent here
+                    // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
+                    ptx::mbar_wait(&sm.pv_done[1][tile], (j - 1) & 1);
+                    ptx::tc_fence_after();
                     const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
                     if (grow) m_used = m_new;
                     const uint64_t alpha2 = ptx::pack2(alpha, alpha);
@@ -245,30 +288,49 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     ptx::tmem_st1(t_o + kD, __float_as_uint(l_old * alpha));
                 }
                 const uint64_t neg_m2 = ptx::pack2(-m_used, -m_used);
+                uint64_t scale_h = scale2;
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+                for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        ptx::ffma2(s[c][i], s[c][i + 1], scale2, neg_m2);
-                        s[c][i] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i])));
-                        s[c][i + 1] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i + 1])));
+                    for (int c = 2 * h; c < 2 * h + 2; ++c) {
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) {
+                            ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
+                            if (((i >> 1) & 15) % 4 == 3 && ((i >> 1) & 15) / 4 < kPolyPairs) {
+                                exp2_poly2(s[c][i], s[c][i + 1]);
+                            } else {
+                                s[c][i] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i])));
+                                s[c][i + 1] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i + 1])));
+                            }
+                        }
                     }
-#pragma unroll
-                for (int c = 0; c < 2; ++c) {
                     uint32_t pk[32];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
-                        pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * c][2 * i]), __uint_as_float(s[2 * c][2 * i + 1]));
-                        pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * c + 1][2 * i]), __uint_as_float(s[2 * c + 1][2 * i + 1]));
+                        pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * h][2 * i]), __uint_as_float(s[2 * h][2 * i + 1]));
+                        pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1]));
                     }
-                    ptx::tmem_st32(t_p + 32 * c, pk);
+                    // the P half buffer is free once the previous PV that read it has completed
+                    if (h == 1) ptx::mbar_wait(&sm.pv_done[0][tile], j & 1);
+                    else if (j > 0) ptx::mbar_wait(&sm.pv_done[1][tile], (j - 1) & 1);
+                    ptx::tc_fence_after();
+                    ptx::tmem_st32(t_p, pk);
+                    ptx::tc_wait_st();
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&sm.p_full[h][tile]);
+                    if (h == 0) {
+                        // Keep the second half's exponentials behind the first half's store (ptxas would hoist them
+                        // above it): their scale operand passes through an opaque shared-memory read of a zero word.
+                        uint32_t z;
+                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(ptx::smem_u32(&sm.zero)) : "memory");
+                        scale_h = ptx::pack2(__uint_as_float(__float_as_uint(prm.scale_log2) | z),
+                                             __uint_as_float(__float_as_uint(prm.scale_log2) | z));
+                    }
                 }
-                ptx::tc_wait_st();
-                ptx::tc_fence_before();
-                ptx::mbar_arrive(&sm.p_full[tile]);
             }
             // ---- epilogue: O / l -> bf16 -> global ----
-            ptx::mbar_wait(&sm.o_final[tile], 0);
+            ptx::mbar_wait(&sm.pv_done[1][tile], (n_kv - 1) & 1);
             ptx::tc_fence_after();
             const int row = row0 + tile * kBM + row_in_tile;
             uint32_t o[2][32];
