@@ -12,19 +12,30 @@
 //                      write M = U/Z and G = M*D (128-bit, streaming stores).  12 B/pixel.
 #include "common.h"
 
+#include <algorithm>
 #include <cfloat>
+#include <climits>
 #include <cmath>
 
 namespace mf {
 
 constexpr int kMaxPoints = 32;
 constexpr int kTile = 32;                 // branch-and-bound tile edge (pixels)
+#ifndef MF_NORM_BLOCKS
+#define MF_NORM_BLOCKS 8
+#endif
+constexpr int kNormBlocks = MF_NORM_BLOCKS;            // CTAs per frame in norm_kernel (MF_NORM_MAX tiles are dealt round-robin)
+constexpr double kTruncate = 34.5;         // separable factors below e^-34.5 = 1e-15 of their peak are stored as 0
+constexpr float kCullBelow = 1e-13f;      // a column factor below this adds < 1e-13 of the map's peak (S8(c)-D3 allows 1e-12)
 
 struct FrameMeta {
     int n_valid;
-    float inv_z;        // 1/Z' of the rescaled map
+    float inv_z;        // 1/Z' of the rescaled map (MF_NORM_SUM, MF_NORM_NONE)
     float out_scale;    // exp(cmax): only applied for MF_NORM_NONE
-    int pad;
+    int pad;            // 1: the whole frame underflows in fp64 (renders as zero)
+    unsigned zmax_bits; // MF_NORM_MAX: bit pattern of Z' = max U' (>= 0, so unsigned order == float order)
+    int xa, xb, ya, yb; // columns [xa,xb] x rows [ya,yb]: outside it every point's separable factor is < kCullBelow
+    int reserved[7];
 };
 
 struct Workspace {
@@ -76,13 +87,13 @@ __device__ __forceinline__ double norm3(const double a[3]) {
     return __dsqrt_rn(dadd(dadd(dmul(a[0], a[0]), dmul(a[1], a[1])), dmul(a[2], a[2])));
 }
 
-__global__ void __launch_bounds__(128)
-points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict__ pts, FrameMeta* __restrict__ meta,
-              float* __restrict__ focus_uv, int32_t* __restrict__ focus_index) {
-    // one warp per rendered frame; lane = slot in the trailing window (oldest first), n_points <= 32
-    const int f = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (f >= pp.count) return;
+// Eq. 1-6 for rendered frame f by one full warp; lane = slot in the trailing window (oldest first), n_points <= 32.
+// The valid points are compacted into spts[0..n_valid) (shared memory, (u, v, sigma, 0) rounded once to fp32);
+// with `write` they, n_valid, focus_uv and focus_index also go to global memory.  Returns n_valid.
+__device__ __forceinline__ int frame_points_warp(const double* __restrict__ w2c, const PointParams& pp, int f, int lane,
+                                                 float4* spts, bool write, float4* __restrict__ pts,
+                                                 FrameMeta* __restrict__ meta, float* __restrict__ focus_uv,
+                                                 int32_t* __restrict__ focus_index) {
     const int t = pp.render_begin + f;
     const int i = t - pp.n_points + 1 + lane;
     const int need = pp.vec == MF_VEC_ACCEL ? 2 : 1;
@@ -115,10 +126,20 @@ points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
         if (sig < 1e-3) sig = 1e-3;
     }
     const unsigned mask = __ballot_sync(0xffffffffu, valid);
-    if (valid)
-        pts[static_cast<size_t>(f) * kMaxPoints + __popc(mask & ((1u << lane) - 1u))] =
-            make_float4(__double2float_rn(u), __double2float_rn(v), __double2float_rn(sig), 0.f);
-    if (lane == 0) meta[f].n_valid = __popc(mask);
+    const int n_valid = __popc(mask);
+    if (valid) {
+        const float4 q = make_float4(__double2float_rn(u), __double2float_rn(v), __double2float_rn(sig), 0.f);
+        const int slot = __popc(mask & ((1u << lane) - 1u));
+        spts[slot] = q;
+        if (write) pts[static_cast<size_t>(f) * kMaxPoints + slot] = q;
+    }
+    __syncwarp();
+    if (!write) return n_valid;
+    if (lane == 0) {
+        meta[f].n_valid = n_valid;
+        meta[f].zmax_bits = 0u;
+        meta[f].xa = INT_MAX; meta[f].xb = -1; meta[f].ya = INT_MAX; meta[f].yb = -1;
+    }
     if (lane == pp.n_points - 1) {                      // the frame's own point (i == t)
         int index = -1;
         float fu = __int_as_float(0x7fc00000), fv = __int_as_float(0x7fc00000);
@@ -138,10 +159,21 @@ points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
         }
         if (focus_index) focus_index[f] = index;
     }
+    return n_valid;
+}
+
+// points only (focus_map == NULL): one warp per rendered frame
+__global__ void __launch_bounds__(128)
+points_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict__ pts, FrameMeta* __restrict__ meta,
+              float* __restrict__ focus_uv, int32_t* __restrict__ focus_index) {
+    __shared__ float4 spts[4][kMaxPoints];
+    const int f = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (f >= pp.count) return;
+    frame_points_warp(w2c, pp, f, threadIdx.x & 31, spts[threadIdx.x >> 5], true, pts, meta, focus_uv, focus_index);
 }
 
 // ------------------------------------------------------------------------------------------------
-// 2. separable tables (fp64 evaluation, fp32 storage).  grid = (npad, count), one (frame, slot) each.
+// 2. separable tables (fp64 evaluation, fp32 storage).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double nearest_in_range(double u, int hi) {
     // integer coordinate in [0, hi] nearest to u
@@ -164,52 +196,87 @@ __device__ __forceinline__ double log_peak(float4 p, int width, int height, doub
     return -((*dxmin) * (*dxmin) + (*dymin) * (*dymin)) / (2.0 * s * s);
 }
 
+__device__ __forceinline__ int warp_min_i(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ int warp_max_i(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+struct TablePoint {     // per-point constants of the separable factors (fp64)
+    double u, v, inv, dx0sq, dy0sq, w;
+    int live;
+};
+constexpr int kTableItems = 8;              // table entries per thread
+
+// grid = (chunks, count): a CTA fills kTableItems*256 consecutive entries of the frame's [Ex | EyT] tables, so every
+// store is coalesced; the per-point constants are recomputed by warp 0 of every CTA (15 lanes of fp64, ~1 us).
 __global__ void __launch_bounds__(256)
-tables_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, float* __restrict__ ex,
+tables_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict__ pts, FrameMeta* __restrict__ meta,
+              float* __restrict__ focus_uv, int32_t* __restrict__ focus_index, float* __restrict__ ex,
               float* __restrict__ eyt, int npad, int width, int height) {
-    const int j = blockIdx.x, f = blockIdx.y;
-    const int n_valid = meta[f].n_valid;
-    const float4* fp = pts + static_cast<size_t>(f) * kMaxPoints;
-    // common factor exp(cmax) pulled out of every point of this frame (cancels in U/Z)
-    double cmax = -INFINITY, dx0 = 0.0, dy0 = 0.0, lw_j = -INFINITY;
-    for (int k = 0; k < n_valid; ++k) {
-        double a, b;
-        const double lw = log_peak(fp[k], width, height, &a, &b);
-        cmax = lw > cmax ? lw : cmax;
-        if (k == j) {
-            lw_j = lw;
-            dx0 = a;
-            dy0 = b;
+    __shared__ TablePoint tp[kMaxPoints];
+    __shared__ float4 spts[kMaxPoints];
+    const int f = blockIdx.y;
+    const int lane = threadIdx.x & 31;
+    if (threadIdx.x < 32) {
+        // the frame's motion points (every CTA recomputes them; CTA 0 of the frame publishes them)
+        const int n_valid = frame_points_warp(w2c, pp, f, lane, spts, blockIdx.x == 0, pts, meta, focus_uv, focus_index);
+        // common factor exp(cmax) pulled out of every point of this frame (cancels in U/Z)
+        double dx0 = 0.0, dy0 = 0.0, lw = -INFINITY;
+        float4 p = make_float4(0.f, 0.f, 1.f, 0.f);
+        if (lane < n_valid) {
+            p = spts[lane];
+            lw = log_peak(p, width, height, &dx0, &dy0);
         }
+        double cmax = lw;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cmax = fmax(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
+        const bool frame_empty = !(cmax > -700.0);      // fp64 Eq. 7 underflows to 0 everywhere
+        if (blockIdx.x == 0 && lane == 0) {
+            meta[f].out_scale = frame_empty ? 0.f : static_cast<float>(exp(cmax));
+            meta[f].pad = frame_empty ? 1 : 0;
+        }
+        TablePoint t;
+        const double sg = p.z;
+        t.u = p.x; t.v = p.y; t.inv = 1.0 / (2.0 * sg * sg);
+        t.dx0sq = dx0 * dx0; t.dy0sq = dy0 * dy0;
+        t.live = lane < n_valid && !frame_empty && lw > -INFINITY;
+        t.w = t.live ? exp(lw - cmax) : 0.0;
+        tp[lane] = t;
     }
-    const bool frame_empty = !(cmax > -700.0);          // fp64 Eq. 7 underflows to 0 everywhere
-    if (j == 0 && threadIdx.x == 0) {
-        meta[f].out_scale = frame_empty ? 0.f : static_cast<float>(exp(cmax));
-        meta[f].pad = frame_empty ? 1 : 0;
-    }
-    float* exr = ex + (static_cast<size_t>(f) * npad + j) * width;
-    float* eyc = eyt + static_cast<size_t>(f) * height * npad + j;
-    const bool live = j < n_valid && !frame_empty && lw_j > -INFINITY;
-    if (!live) {
-        for (int x = threadIdx.x; x < width; x += blockDim.x) exr[x] = 0.f;
-        for (int y = threadIdx.x; y < height; y += blockDim.x) eyc[static_cast<size_t>(y) * npad] = 0.f;
-        return;
-    }
-    const double u = fp[j].x, v = fp[j].y, s = fp[j].z;
-    const double inv = 1.0 / (2.0 * s * s);
-    const double w = exp(lw_j - cmax);
-    for (int x = threadIdx.x; x < width; x += blockDim.x) {
-        const double d = static_cast<double>(x) - u;
-        exr[x] = static_cast<float>(exp(-(d * d - dx0 * dx0) * inv));
-    }
-    for (int y = threadIdx.x; y < height; y += blockDim.x) {
-        const double d = static_cast<double>(y) - v;
-        eyc[static_cast<size_t>(y) * npad] = static_cast<float>(w * exp(-(d * d - dy0 * dy0) * inv));
+    __syncthreads();
+    const int n_ex = npad * width, n_all = n_ex + npad * height;
+    float* exf = ex + static_cast<size_t>(f) * n_ex;
+    float* eyf = eyt + static_cast<size_t>(f) * height * npad;
+#pragma unroll
+    for (int it = 0; it < kTableItems; ++it) {
+        const int idx = (blockIdx.x * kTableItems + it) * 256 + threadIdx.x;
+        if (idx < n_ex) {
+            const int j = idx / width, x = idx - j * width;
+            const TablePoint& t = tp[j];
+            const double d = static_cast<double>(x) - t.u;
+            const double a = (d * d - t.dx0sq) * t.inv;
+            const float val = (!t.live || a > kTruncate) ? 0.f : static_cast<float>(exp(-a));
+            exf[idx] = val;
+        } else if (idx < n_all) {
+            const int i = idx - n_ex;
+            const int y = i / npad, j = i - y * npad;
+            const TablePoint& t = tp[j];
+            const double d = static_cast<double>(y) - t.v;
+            const double a = (d * d - t.dy0sq) * t.inv;
+            const float val = (!t.live || a > kTruncate) ? 0.f : static_cast<float>(t.w * exp(-a));
+            eyf[i] = val;
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// 3. per-frame normaliser.  grid = count, 256 threads, dynamic smem = npad*(TC+TR) floats.
+// 3. per-frame normaliser.  grid = (kNormBlocks, count), 256 threads, dynamic smem = npad*(TC+TR) floats.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
@@ -221,28 +288,78 @@ __device__ __forceinline__ int clamp_round(float u, int lo, int hi) {
     return static_cast<int>(fminf(fmaxf(rintf(u), static_cast<float>(lo)), static_cast<float>(hi)));
 }
 
-// U'(x,y) with the SAME fma chain as render_kernel (so that max M == Zmax * inv_z)
-__device__ __forceinline__ float eval_pixel(const float* __restrict__ exf, const float* __restrict__ eyrow,
-                                            int npad, int width, int x) {
-    float acc = 0.f;
-    for (int k = 0; k < npad; ++k) acc = fmaf(exf[static_cast<size_t>(k) * width + x], eyrow[k], acc);
-    return acc;
+constexpr int kMaxSurvivors = 256;
+
+// Largest U'(x,y) over one kTile x kTile tile, lane = column, with the SAME fma chain (k ascending) as render_kernel.
+// The tile's row factors (contiguous in EyT) are staged in shared memory by the warp: every global load of the tile
+// is in flight at once.
+__device__ __forceinline__ float eval_tile(const float* __restrict__ exf, const float* __restrict__ eyf, float* buf, int npad,
+                                           int width, int height, int tile, int tc, int lane) {
+    const int c = tile % tc, r = tile / tc;
+    const int x = min(c * kTile + lane, width - 1);                         // duplicates are harmless for a max
+    const int y0 = r * kTile, rows = min(y0 + kTile, height) - y0;
+    float e[kMaxPoints];
+#pragma unroll
+    for (int k = 0; k < kMaxPoints; ++k) e[k] = k < npad ? __ldg(exf + static_cast<size_t>(k) * width + x) : 0.f;
+    const float4* src = reinterpret_cast<const float4*>(eyf + static_cast<size_t>(y0) * npad);
+    const int n4 = rows * npad / 4;
+    float4 stage[kTile * kMaxPoints / 4 / 32];
+#pragma unroll
+    for (int u = 0; u < kTile * kMaxPoints / 4 / 32; ++u)
+        if (u * 32 + lane < n4) stage[u] = __ldg(src + u * 32 + lane);
+    __syncwarp();                                                           // previous tile's readers are done
+#pragma unroll
+    for (int u = 0; u < kTile * kMaxPoints / 4 / 32; ++u)
+        if (u * 32 + lane < n4) reinterpret_cast<float4*>(buf)[u * 32 + lane] = stage[u];
+    __syncwarp();
+    float local = 0.f;
+    for (int y = 0; y < rows; ++y) {
+        const float* row = buf + y * npad;
+        float acc = 0.f;
+#pragma unroll
+        for (int k = 0; k < kMaxPoints; ++k)
+            if (k < npad) acc = fmaf(e[k], row[k], acc);
+        local = fmaxf(local, acc);
+    }
+    return local;
 }
 
 __global__ void __launch_bounds__(256)
 norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const float* __restrict__ ex,
             const float* __restrict__ eyt, int npad, int width, int height, int norm) {
     extern __shared__ float sm_f[];
-    __shared__ float s_red[8];
     __shared__ double s_dred[8];
-    const int f = blockIdx.x;
+    const int f = blockIdx.y, part = blockIdx.x;
     const int n_valid = meta[f].n_valid;
+    if (part != 0 && (norm != MF_NORM_MAX || n_valid == 0 || meta[f].pad != 0)) return;
     const float* exf = ex + static_cast<size_t>(f) * npad * width;
     const float* eyf = eyt + static_cast<size_t>(f) * height * npad;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (n_valid == 0 || meta[f].pad != 0) {
         if (threadIdx.x == 0) meta[f].inv_z = 0.f;
         return;
+    }
+    __shared__ int s_box[4];                // xa, xb, ya, yb of the frame's non-negligible region
+    if (threadIdx.x == 0) {
+        s_box[0] = INT_MAX; s_box[1] = -1; s_box[2] = INT_MAX; s_box[3] = -1;
+    }
+    __syncthreads();
+    if (norm != MF_NORM_MAX) {
+        // bounding box straight from the tables (these modes are not latency-critical)
+        int lo = INT_MAX, hi = -1;
+        for (int x = threadIdx.x; x < width; x += blockDim.x)
+            for (int j = 0; j < n_valid; ++j)
+                if (exf[static_cast<size_t>(j) * width + x] >= kCullBelow) { lo = min(lo, x); hi = max(hi, x); }
+        if (hi >= 0) { atomicMin(&s_box[0], lo); atomicMax(&s_box[1], hi); }
+        lo = INT_MAX; hi = -1;
+        for (int y = threadIdx.x; y < height; y += blockDim.x)
+            for (int j = 0; j < n_valid; ++j)
+                if (eyf[static_cast<size_t>(y) * npad + j] >= kCullBelow) { lo = min(lo, y); hi = max(hi, y); }
+        if (hi >= 0) { atomicMin(&s_box[2], lo); atomicMax(&s_box[3], hi); }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            meta[f].xa = s_box[0]; meta[f].xb = s_box[1]; meta[f].ya = s_box[2]; meta[f].yb = s_box[3];
+        }
     }
     if (norm == MF_NORM_NONE) {
         if (threadIdx.x == 0) meta[f].inv_z = meta[f].out_scale;
@@ -276,90 +393,135 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
         return;
     }
     // ---- MF_NORM_MAX ----
+    // Exact branch and bound.  Every step issues all of its (independent) global loads before using any of them:
+    // the kernel is a chain of memory latencies, not of arithmetic.
     const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
     float* mx = sm_f;                       // [npad][tc] max over the tile's columns of Ex_j
     float* my = sm_f + npad * tc;           // [npad][tr]
-    const float4* fp = pts + static_cast<size_t>(f) * kMaxPoints;
-    for (int i = threadIdx.x; i < npad * tc; i += blockDim.x) {
-        const int j = i / tc, c = i % tc;
-        float val = 0.f;
-        if (j < n_valid) {
-            const int x0 = c * kTile, x1 = min(x0 + kTile, width) - 1;
-            val = exf[static_cast<size_t>(j) * width + clamp_round(fp[j].x, x0, x1)];
-        }
-        mx[i] = val;
-    }
-    for (int i = threadIdx.x; i < npad * tr; i += blockDim.x) {
-        const int j = i / tr, r = i % tr;
-        float val = 0.f;
-        if (j < n_valid) {
-            const int y0 = r * kTile, y1 = min(y0 + kTile, height) - 1;
-            val = eyf[static_cast<size_t>(clamp_round(fp[j].y, y0, y1)) * npad + j];
-        }
-        my[i] = val;
-    }
-    // lower bound: the map at the pixel nearest to each centre
-    float best = 0.f;
-    if (warp == 0) {
-        if (lane < n_valid) {
-            const int x = clamp_round(fp[lane].x, 0, width - 1), y = clamp_round(fp[lane].y, 0, height - 1);
-            best = eval_pixel(exf, eyf + static_cast<size_t>(y) * npad, npad, width, x);
-        }
-        best = warp_max(best);
-        if (lane == 0) s_red[0] = best;
-    }
-    __syncthreads();
-    best = s_red[0];
-    __syncthreads();
-    // each lane bounds one tile; surviving tiles are then evaluated by the whole warp
-    const int n_tiles = tc * tr;
-    for (int base = warp * 32; base < n_tiles; base += 8 * 32) {
-        const int mine = base + lane;
-        float ub = 0.f;
-        if (mine < n_tiles) {
-            const int c = mine % tc, r = mine / tc;
-            for (int k = 0; k < npad; ++k) ub = fmaf(mx[k * tc + c], my[k * tr + r], ub);
-        } else {
-            ub = -1.f;
-        }
-        unsigned surv = __ballot_sync(0xffffffffu, ub * 1.00001f >= best);
-        while (surv) {
-            const int src = __ffs(surv) - 1;
-            surv &= surv - 1;
-            if (__shfl_sync(0xffffffffu, ub, src) * 1.00001f < best) continue;     // best may have grown
-            const int tile = base + src;
-            const int c = tile % tc, r = tile / tc;
-            const int x = min(c * kTile + lane, width - 1);                         // duplicates are harmless for a max
-            const int y0 = r * kTile, y1 = min(y0 + kTile, height);
-            float local = 0.f;
-            float e[kMaxPoints];
-#pragma unroll
-            for (int k = 0; k < kMaxPoints; ++k) e[k] = k < npad ? exf[static_cast<size_t>(k) * width + x] : 0.f;
-            for (int y = y0; y < y1; ++y) {
-                const float4* row = reinterpret_cast<const float4*>(eyf + static_cast<size_t>(y) * npad);
-                float acc = 0.f;
-#pragma unroll
-                for (int q = 0; q < kMaxPoints / 4; ++q) {
-                    if (4 * q < npad) {
-                        const float4 w = __ldg(row + q);
-                        acc = fmaf(e[4 * q + 0], w.x, acc);
-                        acc = fmaf(e[4 * q + 1], w.y, acc);
-                        acc = fmaf(e[4 * q + 2], w.z, acc);
-                        acc = fmaf(e[4 * q + 3], w.w, acc);
-                    }
-                }
-                local = fmaxf(local, acc);
-            }
-            best = fmaxf(best, warp_max(local));
-        }
-    }
-    if (lane == 0) s_red[warp] = best;
-    __syncthreads();
+    __shared__ float4 s_pts[kMaxPoints];
+    __shared__ unsigned s_best;             // bit pattern of a lower bound of the frame's maximum
+    __shared__ unsigned s_exact;            // bit pattern of the largest exactly evaluated pixel of this CTA
+    __shared__ int s_count;
+    __shared__ int s_list[kMaxSurvivors];
+    if (threadIdx.x < kMaxPoints)
+        s_pts[threadIdx.x] = threadIdx.x < n_valid ? pts[static_cast<size_t>(f) * kMaxPoints + threadIdx.x]
+                                                   : make_float4(0.f, 0.f, 1.f, 0.f);
+    float* centre = sm_f + npad * (tc + tr);                    // [kMaxPoints] map value at each centre's pixel
+    float* tile_buf = centre + kMaxPoints;                      // [8 warps][kTile rows][kMaxPoints] staged row factors
+    if (threadIdx.x < kMaxPoints) centre[threadIdx.x] = 0.f;
     if (threadIdx.x == 0) {
-        float z = 0.f;
-        for (int w = 0; w < 8; ++w) z = fmaxf(z, s_red[w]);
-        meta[f].inv_z = z > 0.f ? 1.0f / z : 0.f;
+        s_best = 0u;
+        s_exact = 0u;
+        s_count = 0;
     }
+    __syncthreads();
+    constexpr int kPer = 8;                 // table entries per thread and pass
+    for (int base = 0; base < npad * tc; base += kPer * 256) {
+        float val[kPer];
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int i = base + u * 256 + threadIdx.x;
+            const int j = i / tc, c = i - j * tc;
+            val[u] = 0.f;
+            if (i < npad * tc && j < n_valid) {
+                const int x0 = c * kTile, x1 = min(x0 + kTile, width) - 1;
+                val[u] = __ldg(exf + static_cast<size_t>(j) * width + clamp_round(s_pts[j].x, x0, x1));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int i = base + u * 256 + threadIdx.x;
+            if (i < npad * tc) mx[i] = val[u];
+        }
+    }
+    for (int base = 0; base < npad * tr; base += kPer * 256) {
+        float val[kPer];
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int i = base + u * 256 + threadIdx.x;
+            const int j = i / tr, r = i - j * tr;
+            val[u] = 0.f;
+            if (i < npad * tr && j < n_valid) {
+                const int y0 = r * kTile, y1 = min(y0 + kTile, height) - 1;
+                val[u] = __ldg(eyf + static_cast<size_t>(clamp_round(s_pts[j].y, y0, y1)) * npad + j);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int i = base + u * 256 + threadIdx.x;
+            if (i < npad * tr) my[i] = val[u];
+        }
+    }
+    // lower bound: the map at the pixel nearest to each centre; one (centre p, term k) product per thread, summed over k
+    // in any order (a bound, not the result: the tile holding that pixel is evaluated exactly below)
+    for (int base = 0; base < n_valid * npad; base += 256) {
+        const int i = base + threadIdx.x;
+        float term = 0.f;
+        if (i < n_valid * npad) {
+            const int p = i / npad, k = i - p * npad;
+            const int x = clamp_round(s_pts[p].x, 0, width - 1), y = clamp_round(s_pts[p].y, 0, height - 1);
+            term = __ldg(exf + static_cast<size_t>(k) * width + x) * __ldg(eyf + static_cast<size_t>(y) * npad + k);
+        }
+        // npad is 8, 16, 24 or 32: groups of 8 lanes never straddle two centres
+        term += __shfl_xor_sync(0xffffffffu, term, 1);
+        term += __shfl_xor_sync(0xffffffffu, term, 2);
+        term += __shfl_xor_sync(0xffffffffu, term, 4);
+        if ((lane & 7) == 0 && i < n_valid * npad) atomicAdd(&centre[i / npad], term);
+    }
+    __syncthreads();
+    if (threadIdx.x < n_valid) atomicMax(&s_best, __float_as_uint(fmaxf(centre[threadIdx.x], 0.f) * 0.9999f));
+    if (part == 0) {
+        // bounding box at tile granularity: mx / my hold each point's largest factor per tile column / row
+        for (int i = threadIdx.x; i < tc + tr; i += blockDim.x) {
+            const bool col = i < tc;
+            const int t = col ? i : i - tc;
+            bool any = false;
+            for (int j = 0; j < n_valid; ++j) any |= (col ? mx[j * tc + t] : my[j * tr + t]) >= kCullBelow;
+            if (any) {
+                atomicMin(&s_box[col ? 0 : 2], t * kTile);
+                atomicMax(&s_box[col ? 1 : 3], min(t * kTile + kTile, col ? width : height) - 1);
+            }
+        }
+    }
+    __syncthreads();
+    if (part == 0 && threadIdx.x == 0) {
+        meta[f].xa = s_box[0]; meta[f].xb = s_box[1]; meta[f].ya = s_box[2]; meta[f].yb = s_box[3];
+    }
+    const float best = __uint_as_float(s_best);
+    float exact = 0.f;
+    // tile t belongs to warp (t mod 8*kNormBlocks) of the frame: neighbouring (surviving) tiles go to different warps
+    constexpr int kWarpsPerFrame = 8 * kNormBlocks;
+    const int gw = part * 8 + warp;
+    const int n_tiles = tc * tr;
+    for (int i = lane; i * kWarpsPerFrame + gw < n_tiles; i += 32) {
+        const int tile = i * kWarpsPerFrame + gw;
+        const int c = tile % tc, r = tile / tc;
+        float ub = 0.f;
+        for (int k = 0; k < npad; ++k) ub = fmaf(mx[k * tc + c], my[k * tr + r], ub);
+        if (ub * 1.00001f >= best) {
+            const int slot = atomicAdd(&s_count, 1);
+            if (slot < kMaxSurvivors) s_list[slot] = tile;
+        }
+    }
+    __syncthreads();
+    const int n_surv = s_count;
+    if (n_surv > kMaxSurvivors) {
+        // more survivors than the list holds (huge sigma): fall back to this CTA's whole share of the tiles
+        for (int i = warp; i * kNormBlocks + part < n_tiles; i += 8) {
+            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
+                                                    i * kNormBlocks + part, tc, lane)));
+        }
+    } else {
+        for (int i = warp; i < n_surv; i += 8) {
+            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
+                                                    s_list[i], tc, lane)));
+        }
+    }
+    // only exactly evaluated pixels may set Z (the bound above is 0.9999 x an approximately summed value); the tile
+    // holding the true maximum always survives: its bound is >= the map's value there >= every centre value >= best
+    if (lane == 0) atomicMax(&s_exact, __float_as_uint(exact));
+    __syncthreads();
+    if (threadIdx.x == 0 && s_exact != 0u) atomicMax(&meta[f].zmax_bits, s_exact);      // order-independent: deterministic
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -368,8 +530,20 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
 //    of each row are a broadcast 128-bit read of EyT (L1-resident).  Algorithmic HBM traffic is
 //    12 B/pixel with depth and guided depth, 4 B/pixel map-only.
 // ------------------------------------------------------------------------------------------------
-constexpr int kRowsPerThread = 32;
-constexpr int kRenderThreads = 256;
+#ifndef MF_RENDER_ROWS
+#define MF_RENDER_ROWS 32
+#endif
+#ifndef MF_RENDER_THREADS
+#define MF_RENDER_THREADS 256
+#endif
+#ifndef MF_RENDER_U
+#define MF_RENDER_U 4
+#endif
+#ifndef MF_RENDER_MINB
+#define MF_RENDER_MINB 1
+#endif
+constexpr int kRowsPerThread = MF_RENDER_ROWS;
+constexpr int kRenderThreads = MF_RENDER_THREADS;
 
 __device__ __forceinline__ float4 ld_stream(const float4* p) {
     float4 r;
@@ -381,11 +555,37 @@ __device__ __forceinline__ void st_stream(float4* p, float4 v) {
     asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
+// rows [ya, yb) of this thread's 4 columns where the map is identically zero: M = 0, G = 0 * D (depth is still read)
+template <bool HAS_DEPTH, bool HAS_G>
+__device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth, float* __restrict__ focus_map,
+                                                 float* __restrict__ guided, size_t img, int width, int ya, int yb) {
+    constexpr int U = 8;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int y = ya; y < yb; y += U) {
+        float4 d[U];
+        if (HAS_G) {
+#pragma unroll
+            for (int r = 0; r < U; ++r)
+                if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
+        }
+#pragma unroll
+        for (int r = 0; r < U; ++r) {
+            if (y + r < yb) {
+                const size_t o = img + static_cast<size_t>(y + r) * width;
+                st_stream(reinterpret_cast<float4*>(focus_map + o), zero);
+                if (HAS_G)
+                    st_stream(reinterpret_cast<float4*>(guided + o),
+                              make_float4(0.f * d[r].x, 0.f * d[r].y, 0.f * d[r].z, 0.f * d[r].w));
+            }
+        }
+    }
+}
+
 template <int NP, bool HAS_DEPTH, bool HAS_G>
-__global__ void __launch_bounds__(kRenderThreads)
+__global__ void __launch_bounds__(kRenderThreads, MF_RENDER_MINB)
 render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const FrameMeta* __restrict__ meta,
               const float* __restrict__ depth, float* __restrict__ focus_map, float* __restrict__ guided,
-              int width, int height, int blocks_per_frame) {
+              int width, int height, int blocks_per_frame, int norm) {
     const int f = blockIdx.x / blocks_per_frame;
     const int b = blockIdx.x - f * blocks_per_frame;
     const int wq = width >> 2;
@@ -393,65 +593,89 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
     const int rb = idx / wq;
     const int x = (idx - rb * wq) << 2;
     const int y0 = rb * kRowsPerThread;
-    if (y0 >= height) return;
-    const int y1 = min(y0 + kRowsPerThread, height);
-    const float scale = meta[f].inv_z;
-
-    float4 e[NP];
-    const float* exf = ex + static_cast<size_t>(f) * NP * width + x;
-#pragma unroll
-    for (int j = 0; j < NP; ++j) e[j] = __ldg(reinterpret_cast<const float4*>(exf + static_cast<size_t>(j) * width));
-
+    if (__all_sync(0xffffffffu, y0 >= height)) return;          // whole warp past the image
+    const int y1 = max(y0, min(y0 + kRowsPerThread, height));    // == y0 for a lane past the image: no rows
+    const FrameMeta fm = meta[f];
+    float scale = fm.inv_z;
+    if (norm == MF_NORM_MAX) {
+        const float z = __uint_as_float(fm.zmax_bits);
+        scale = z > 0.f ? 1.0f / z : 0.f;
+    }
     const size_t img = static_cast<size_t>(f) * height * width + x;
-    const float4* eyrow = reinterpret_cast<const float4*>(eyt + (static_cast<size_t>(f) * height + y0) * NP);
-    constexpr int U = 4;
-    for (int y = y0; y < y1; y += U) {
-        float4 d[U];
-        if (HAS_DEPTH) {
+
+    // Outside columns [xa,xb] x rows [ya,yb] every term of Eq. 7 is below kCullBelow of the map's peak (S8(c)-D3):
+    // those pixels are written as exact zeros by a pure streaming loop.  The test is warp-uniform.
+    const bool cols_hit = x + 3 >= fm.xa && x <= fm.xb && y1 > y0;
+    const bool warp_live = __any_sync(0xffffffffu, cols_hit) && scale != 0.f;
+    const int ya = warp_live ? min(max(fm.ya, y0), y1) : y1;     // live rows of this thread: [ya, yb)
+    const int yb = warp_live ? min(max(fm.yb + 1, ya), y1) : y1;
+    stream_zero_rows<HAS_DEPTH, HAS_G>(depth, focus_map, guided, img, width, y0, ya);
+    if (__any_sync(0xffffffffu, ya < yb)) {
+        float4 e[NP];
+        const float* exf = ex + static_cast<size_t>(f) * NP * width + x;
 #pragma unroll
-            for (int r = 0; r < U; ++r)
-                if (y + r < y1) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
+        for (int j = 0; j < NP; ++j) e[j] = __ldg(reinterpret_cast<const float4*>(exf + static_cast<size_t>(j) * width));
+        // groups of 4 points whose column factors are negligible over all of this warp's columns are skipped
+        unsigned live = 0u;
+#pragma unroll
+        for (int q = 0; q < NP / 4; ++q) {
+            float m = 0.f;
+#pragma unroll
+            for (int k = 4 * q; k < 4 * q + 4; ++k) m = fmaxf(m, fmaxf(fmaxf(e[k].x, e[k].y), fmaxf(e[k].z, e[k].w)));
+            if (__any_sync(0xffffffffu, m >= kCullBelow && ya < yb)) live |= 1u << q;
         }
+        const float4* eyrow = reinterpret_cast<const float4*>(eyt + static_cast<size_t>(f) * height * NP);
+        constexpr int U = MF_RENDER_U;
+        for (int y = ya; y < yb; y += U) {
+            float4 d[U];
+            if (HAS_DEPTH) {
 #pragma unroll
-        for (int r = 0; r < U; ++r) {
-            if (y + r < y1) {
-                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int r = 0; r < U; ++r)
+                    if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
+            }
 #pragma unroll
-                for (int q = 0; q < NP / 4; ++q) {
-                    const float4 w = __ldg(eyrow + (y - y0 + r) * (NP / 4) + q);
-                    const float wy[4] = {w.x, w.y, w.z, w.w};
+            for (int r = 0; r < U; ++r) {
+                if (y + r < yb) {
+                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        acc.x = fmaf(e[4 * q + k].x, wy[k], acc.x);
-                        acc.y = fmaf(e[4 * q + k].y, wy[k], acc.y);
-                        acc.z = fmaf(e[4 * q + k].z, wy[k], acc.z);
-                        acc.w = fmaf(e[4 * q + k].w, wy[k], acc.w);
+                    for (int q = 0; q < NP / 4; ++q) {
+                        if (!(live & (1u << q))) continue;
+                        const float4 w = __ldg(eyrow + static_cast<size_t>(y + r) * (NP / 4) + q);
+                        const float wy[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            acc.x = fmaf(e[4 * q + k].x, wy[k], acc.x);
+                            acc.y = fmaf(e[4 * q + k].y, wy[k], acc.y);
+                            acc.z = fmaf(e[4 * q + k].z, wy[k], acc.z);
+                            acc.w = fmaf(e[4 * q + k].w, wy[k], acc.w);
+                        }
                     }
+                    const float4 m = make_float4(acc.x * scale, acc.y * scale, acc.z * scale, acc.w * scale);
+                    const size_t o = img + static_cast<size_t>(y + r) * width;
+                    st_stream(reinterpret_cast<float4*>(focus_map + o), m);
+                    if (HAS_G)
+                        st_stream(reinterpret_cast<float4*>(guided + o),
+                                  make_float4(m.x * d[r].x, m.y * d[r].y, m.z * d[r].z, m.w * d[r].w));
                 }
-                const float4 m = make_float4(acc.x * scale, acc.y * scale, acc.z * scale, acc.w * scale);
-                const size_t o = img + static_cast<size_t>(y + r) * width;
-                st_stream(reinterpret_cast<float4*>(focus_map + o), m);
-                if (HAS_G)
-                    st_stream(reinterpret_cast<float4*>(guided + o),
-                              make_float4(m.x * d[r].x, m.y * d[r].y, m.z * d[r].z, m.w * d[r].w));
             }
         }
     }
+    stream_zero_rows<HAS_DEPTH, HAS_G>(depth, focus_map, guided, img, width, yb, y1);
 }
 
 template <int NP>
 static void launch_render(const Workspace& ws, const float* depth, float* focus_map, float* guided, int count,
-                          int width, int height, cudaStream_t stream) {
+                          int width, int height, int norm, cudaStream_t stream) {
     const int row_blocks = (height + kRowsPerThread - 1) / kRowsPerThread;
     const long long threads = static_cast<long long>(width / 4) * row_blocks;
     const int bpf = static_cast<int>((threads + kRenderThreads - 1) / kRenderThreads);
     const unsigned grid = static_cast<unsigned>(bpf) * static_cast<unsigned>(count);
     if (guided)
         render_kernel<NP, true, true><<<grid, kRenderThreads, 0, stream>>>(ws.ex, ws.eyt, ws.meta, depth, focus_map,
-                                                                            guided, width, height, bpf);
+                                                                            guided, width, height, bpf, norm);
     else
         render_kernel<NP, false, false><<<grid, kRenderThreads, 0, stream>>>(ws.ex, ws.eyt, ws.meta, depth, focus_map,
-                                                                              guided, width, height, bpf);
+                                                                              guided, width, height, bpf, norm);
 }
 
 }  // namespace mf
@@ -500,26 +724,57 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
     pp.eps_z = params->eps_z;
     pp.sigma = static_cast<double>(params->sigma);
     pp.n_points = params->n_points; pp.vec = params->vec; pp.mag = params->mag; pp.pts = params->pts;
-    pp.width = width; pp.height = height; pp.render_begin = render_begin; pp.count = count;
-    points_kernel<<<(count + 3) / 4, 128, 0, s>>>(global_w2c, pp, ws.pts, ws.meta, focus_uv, focus_index);
-    MF_CUDA_OK(cudaGetLastError());
-    if (!focus_map) return MF_OK;
+    pp.width = width; pp.height = height;
 
-    tables_kernel<<<dim3(npad, count), 256, 0, s>>>(ws.pts, ws.meta, ws.ex, ws.eyt, npad, width, height);
-    MF_CUDA_OK(cudaGetLastError());
     const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
-    const size_t smem = sizeof(float) * npad * static_cast<size_t>(tc + tr);
-    if (smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
-    if (smem > 48 * 1024)
-        MF_CUDA_OK(cudaFuncSetAttribute(norm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-    norm_kernel<<<count, 256, smem, s>>>(ws.pts, ws.meta, ws.ex, ws.eyt, npad, width, height, params->norm);
-    MF_CUDA_OK(cudaGetLastError());
-    switch (npad) {
-        case 8: launch_render<8>(ws, depth, focus_map, guided_depth, count, width, height, s); break;
-        case 16: launch_render<16>(ws, depth, focus_map, guided_depth, count, width, height, s); break;
-        case 24: launch_render<24>(ws, depth, focus_map, guided_depth, count, width, height, s); break;
-        default: launch_render<32>(ws, depth, focus_map, guided_depth, count, width, height, s); break;
+    const size_t smem = sizeof(float) * (npad * static_cast<size_t>(tc + tr) + kMaxPoints + 8 * kTile * kMaxPoints);
+    if (focus_map) {
+        if (smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
+        if (smem > 48 * 1024)
+            MF_CUDA_OK(cudaFuncSetAttribute(norm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     }
-    MF_CUDA_OK(cudaGetLastError());
+    const size_t img = static_cast<size_t>(width) * height;
+
+    // points + tables + normaliser of frames [f0, f0+n) (small, latency-bound launches)
+    auto prepare = [&](int f0, int n, cudaStream_t q) -> cudaError_t {
+        PointParams g = pp;
+        g.render_begin = render_begin + f0;
+        g.count = n;
+        float* uv = focus_uv ? focus_uv + 2 * static_cast<size_t>(f0) : nullptr;
+        int32_t* fi = focus_index ? focus_index + f0 : nullptr;
+        if (!focus_map) {
+            points_kernel<<<(n + 3) / 4, 128, 0, q>>>(global_w2c, g, ws.pts + static_cast<size_t>(f0) * kMaxPoints,
+                                                     ws.meta + f0, uv, fi);
+            return cudaGetLastError();
+        }
+        float* ex = ws.ex + static_cast<size_t>(f0) * npad * width;
+        float* eyt = ws.eyt + static_cast<size_t>(f0) * height * npad;
+        const int chunks = (npad * (width + height) + kTableItems * 256 - 1) / (kTableItems * 256);
+        tables_kernel<<<dim3(chunks, n), 256, 0, q>>>(global_w2c, g, ws.pts + static_cast<size_t>(f0) * kMaxPoints, ws.meta + f0,
+                                                      uv, fi, ex, eyt, npad, width, height);
+        norm_kernel<<<dim3(kNormBlocks, n), 256, smem, q>>>(ws.pts + static_cast<size_t>(f0) * kMaxPoints, ws.meta + f0, ex, eyt,
+                                                            npad, width, height, params->norm);
+        return cudaGetLastError();
+    };
+    // the HBM-bound pass over frames [f0, f0+n)
+    auto render = [&](int f0, int n, cudaStream_t q) -> cudaError_t {
+        Workspace w = ws;
+        w.meta = ws.meta + f0;
+        w.ex = ws.ex + static_cast<size_t>(f0) * npad * width;
+        w.eyt = ws.eyt + static_cast<size_t>(f0) * height * npad;
+        const float* d = depth ? depth + f0 * img : nullptr;
+        float* m = focus_map + f0 * img;
+        float* gd = guided_depth ? guided_depth + f0 * img : nullptr;
+        switch (npad) {
+            case 8: launch_render<8>(w, d, m, gd, n, width, height, params->norm, q); break;
+            case 16: launch_render<16>(w, d, m, gd, n, width, height, params->norm, q); break;
+            case 24: launch_render<24>(w, d, m, gd, n, width, height, params->norm, q); break;
+            default: launch_render<32>(w, d, m, gd, n, width, height, params->norm, q); break;
+        }
+        return cudaGetLastError();
+    };
+
+    MF_CUDA_OK(prepare(0, count, s));
+    if (focus_map) MF_CUDA_OK(render(0, count, s));
     return MF_OK;
 }
