@@ -29,7 +29,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = campus, W=32)")
     ap.add_argument("--windows-per-launch", type=int, default=4)
-    ap.add_argument("--focus-chunk", type=int, default=60, help="frames per mf_motion_focus call")
+    ap.add_argument("--focus-chunk", type=int, default=300, help="frames per mf_motion_focus call")
     ap.add_argument("--max-windows", type=int, default=0, help="debug: truncate the clip to this many windows")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

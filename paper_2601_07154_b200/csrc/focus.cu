@@ -1,15 +1,18 @@
-// mf_motion_focus: Eq. 1-7 + motion-guided depth, four launches on the caller's stream:
-//   1. points_kernel   Eq. 1,3,4,6 per rendered frame in fp64 (bit-exact rules of common.h);
-//                      (u_i, v_i, sigma_i) rounded once to fp32, focus_uv / focus_index written.
-//   2. tables_kernel   separable factors of Eq. 7: Ex[f][i][x], EyT[f][y][i] evaluated in fp64,
-//                      stored fp32.  Each point's factors are normalised to peak 1 over the image
-//                      and carry a relative weight w_i <= 1, so far-off-image points cannot
-//                      underflow the whole map (the common factor cancels in M = U/Z).
-//   3. norm_kernel     Z per frame: MAX by an exact branch-and-bound over 32x32 tiles (a tile is
-//                      evaluated only if its separable upper bound can beat the best centre
-//                      value), SUM in closed form from the tables.  Moves no image bytes.
-//   4. render_kernel   the HBM-bound pass: read depth (128-bit), U = sum_i Ex_i[x] EyT[y][i],
-//                      write M = U/Z and G = M*D (128-bit, streaming stores).  12 B/pixel.
+// mf_motion_focus: Eq. 1-7 + motion-guided depth, three launches on the caller's stream (the second and
+// third by programmatic dependent launch):
+//   1. tables_kernel   warp 0 of every CTA: Eq. 1,3,4,6 for the frame's trailing points in fp64 (bit-exact rules of
+//                      common.h), (u_i, v_i, sigma_i) rounded once to fp32; CTA 0 of the frame publishes them with
+//                      focus_uv / focus_index.  Then the separable factors of Eq. 7, Ex[f][i][x] and EyT[f][y][i],
+//                      argument in fp64, stored fp32.  Each point's factors are normalised to peak 1 over the image
+//                      and carry a relative weight w_i <= 1, so far-off-image points cannot underflow the whole map
+//                      (the common factor cancels in M = U/Z).  Factors below 1e-15 of their peak are stored as 0.
+//   2. norm_kernel     Z per frame: MAX by an exact branch-and-bound over 32x32 tiles (a tile is evaluated only if
+//                      its separable upper bound can beat the best centre value), SUM in closed form from the
+//                      tables; also the bounding box outside which every factor is < 1e-13.  Moves no image bytes.
+//   3. render_kernel   the HBM-bound pass: read depth (128-bit), U = sum_i Ex_i[x] EyT[y][i] inside the bounding
+//                      box and exact zeros outside it, write M = U/Z and G = M*D (128-bit, streaming stores).
+//                      12 B/pixel.
+// (points_kernel alone runs when no map is requested.)
 #include "common.h"
 
 #include <algorithm>
@@ -18,6 +21,28 @@
 #include <cmath>
 
 namespace mf {
+
+// Programmatic dependent launch: a kernel launched with launch_pdl() may start while its predecessor on the stream is
+// still running; it must call pdl_wait() before touching anything the predecessor wrote.  pdl_trigger() lets the
+// successor's CTAs be scheduled early (they then sit in pdl_wait()).  This hides launch latency between the short,
+// dependent kernels of one call.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 constexpr int kMaxPoints = 32;
 constexpr int kTile = 32;                 // branch-and-bound tile edge (pixels)
@@ -208,9 +233,20 @@ __device__ __forceinline__ int warp_max_i(int v) {
 }
 
 struct TablePoint {     // per-point constants of the separable factors (fp64)
-    double u, v, inv, dx0sq, dy0sq, w;
+    double u, v, inv, dx0sq, dy0sq, lw;     // lw = log of the point's weight relative to the frame's strongest point (<= 0)
     int live;
 };
+
+// e^-a for 0 <= a <= 40 from an fp64 argument: a*log2(e) = k + r in fp64, 2^-r by ex2.approx on |r| <= 0.5 (fp32,
+// ~2 ulp), 2^-k exactly through the exponent field.  Relative error ~3e-7; exactly 1 at a == 0.
+__device__ __forceinline__ float exp_neg(double a) {
+    const double t = a * 1.4426950408889634;
+    const double k = rint(t);
+    const float r = static_cast<float>(t - k);
+    float p;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p) : "f"(-r));
+    return p * __int_as_float((127 - static_cast<int>(k)) << 23);
+}
 constexpr int kTableItems = 8;              // table entries per thread
 
 // grid = (chunks, count): a CTA fills kTableItems*256 consecutive entries of the frame's [Ex | EyT] tables, so every
@@ -221,6 +257,7 @@ tables_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
               float* __restrict__ eyt, int npad, int width, int height) {
     __shared__ TablePoint tp[kMaxPoints];
     __shared__ float4 spts[kMaxPoints];
+    pdl_trigger();
     const int f = blockIdx.y;
     const int lane = threadIdx.x & 31;
     if (threadIdx.x < 32) {
@@ -246,7 +283,7 @@ tables_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
         t.u = p.x; t.v = p.y; t.inv = 1.0 / (2.0 * sg * sg);
         t.dx0sq = dx0 * dx0; t.dy0sq = dy0 * dy0;
         t.live = lane < n_valid && !frame_empty && lw > -INFINITY;
-        t.w = t.live ? exp(lw - cmax) : 0.0;
+        t.lw = t.live ? lw - cmax : 0.0;
         tp[lane] = t;
     }
     __syncthreads();
@@ -261,15 +298,15 @@ tables_kernel(const double* __restrict__ w2c, PointParams pp, float4* __restrict
             const TablePoint& t = tp[j];
             const double d = static_cast<double>(x) - t.u;
             const double a = (d * d - t.dx0sq) * t.inv;
-            const float val = (!t.live || a > kTruncate) ? 0.f : static_cast<float>(exp(-a));
+            const float val = (!t.live || a > kTruncate) ? 0.f : exp_neg(a);
             exf[idx] = val;
         } else if (idx < n_all) {
             const int i = idx - n_ex;
             const int y = i / npad, j = i - y * npad;
             const TablePoint& t = tp[j];
             const double d = static_cast<double>(y) - t.v;
-            const double a = (d * d - t.dy0sq) * t.inv;
-            const float val = (!t.live || a > kTruncate) ? 0.f : static_cast<float>(t.w * exp(-a));
+            const double a = (d * d - t.dy0sq) * t.inv - t.lw;                // the weight folded into the exponent
+            const float val = (!t.live || a > kTruncate) ? 0.f : exp_neg(a);
             eyf[i] = val;
         }
     }
@@ -329,6 +366,8 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
             const float* __restrict__ eyt, int npad, int width, int height, int norm) {
     extern __shared__ float sm_f[];
     __shared__ double s_dred[8];
+    pdl_wait();                             // tables_kernel's output
+    pdl_trigger();
     const int f = blockIdx.y, part = blockIdx.x;
     const int n_valid = meta[f].n_valid;
     if (part != 0 && (norm != MF_NORM_MAX || n_valid == 0 || meta[f].pad != 0)) return;
@@ -586,6 +625,7 @@ __global__ void __launch_bounds__(kRenderThreads, MF_RENDER_MINB)
 render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const FrameMeta* __restrict__ meta,
               const float* __restrict__ depth, float* __restrict__ focus_map, float* __restrict__ guided,
               int width, int height, int blocks_per_frame, int norm) {
+    pdl_wait();                             // norm_kernel's (and, through it, tables_kernel's) output
     const int f = blockIdx.x / blocks_per_frame;
     const int b = blockIdx.x - f * blocks_per_frame;
     const int wq = width >> 2;
@@ -671,11 +711,11 @@ static void launch_render(const Workspace& ws, const float* depth, float* focus_
     const int bpf = static_cast<int>((threads + kRenderThreads - 1) / kRenderThreads);
     const unsigned grid = static_cast<unsigned>(bpf) * static_cast<unsigned>(count);
     if (guided)
-        render_kernel<NP, true, true><<<grid, kRenderThreads, 0, stream>>>(ws.ex, ws.eyt, ws.meta, depth, focus_map,
-                                                                            guided, width, height, bpf, norm);
+        launch_pdl(render_kernel<NP, true, true>, dim3(grid), dim3(kRenderThreads), 0, stream, ws.ex, ws.eyt, ws.meta, depth,
+                   focus_map, guided, width, height, bpf, norm);
     else
-        render_kernel<NP, false, false><<<grid, kRenderThreads, 0, stream>>>(ws.ex, ws.eyt, ws.meta, depth, focus_map,
-                                                                              guided, width, height, bpf, norm);
+        launch_pdl(render_kernel<NP, false, false>, dim3(grid), dim3(kRenderThreads), 0, stream, ws.ex, ws.eyt, ws.meta,
+                   depth, focus_map, guided, width, height, bpf, norm);
 }
 
 }  // namespace mf
@@ -752,9 +792,10 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
         const int chunks = (npad * (width + height) + kTableItems * 256 - 1) / (kTableItems * 256);
         tables_kernel<<<dim3(chunks, n), 256, 0, q>>>(global_w2c, g, ws.pts + static_cast<size_t>(f0) * kMaxPoints, ws.meta + f0,
                                                       uv, fi, ex, eyt, npad, width, height);
-        norm_kernel<<<dim3(kNormBlocks, n), 256, smem, q>>>(ws.pts + static_cast<size_t>(f0) * kMaxPoints, ws.meta + f0, ex, eyt,
-                                                            npad, width, height, params->norm);
-        return cudaGetLastError();
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        return launch_pdl(norm_kernel, dim3(kNormBlocks, n), dim3(256), smem, q, ws.pts + static_cast<size_t>(f0) * kMaxPoints,
+                          ws.meta + f0, ex, eyt, npad, width, height, static_cast<int>(params->norm));
     };
     // the HBM-bound pass over frames [f0, f0+n)
     auto render = [&](int f0, int n, cudaStream_t q) -> cudaError_t {
