@@ -302,31 +302,21 @@ def main():
         run_reference(args)
         return
     import torch
-    import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2601_07154_b200 import api, replicas
+    rank, local_rank, world = replicas.env_world()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    from paper_2601_07154_b200 import api
+    replicas.init("nccl", dev)
     api.lib()
     peaks = measured_peaks()
     wl = Workload(args.config, args, dev)
     wl.setup_device()
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dev)
 
     def reduce_max(x):
-        if world > 1:
-            t = torch.tensor([x], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-        return x
+        return replicas.max_over_ranks(x, dev)
 
     for _ in range(args.warmup):
         wl.step_device()
@@ -343,7 +333,7 @@ def main():
     clocks = sampler.stop()
     ms_total = reduce_max(e0.elapsed_time(e1))
     ms_step = ms_total / args.steps
-    value = world * wl.N / (ms_step * 1e-3)
+    value = replicas.whole_job_value(wl.N, ms_step, world)
 
     g_ms = sum(a.elapsed_time(b) for a, b, _ in ev_g)
     g_windows = sum(n for _, _, n in ev_g)
@@ -391,8 +381,7 @@ def main():
                 "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
                 "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
         print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finish()
 
 
 if __name__ == "__main__":

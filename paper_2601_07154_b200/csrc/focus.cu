@@ -59,8 +59,7 @@ struct FrameMeta {
     float out_scale;    // exp(cmax): only applied for MF_NORM_NONE
     int pad;            // 1: the whole frame underflows in fp64 (renders as zero)
     unsigned zmax_bits; // MF_NORM_MAX: bit pattern of Z' = max U' (>= 0, so unsigned order == float order)
-    int xa, xb, ya, yb; // columns [xa,xb] x rows [ya,yb]: outside it every point's separable factor is < kCullBelow
-    int reserved[7];
+    int reserved[3];
 };
 
 struct Workspace {
@@ -68,6 +67,8 @@ struct Workspace {
     FrameMeta* meta;    // [count]
     float* ex;          // [count][npad][width]
     float* eyt;         // [count][height][npad]
+    uint32_t* colmask;  // [count][ceil(width/32)]  bit j: point j matters somewhere in this 32-column strip
+    uint32_t* rowmask;  // [count][ceil(height/32)]
 };
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -91,6 +92,11 @@ static size_t carve(void* base, int count, int width, int height, int n_points, 
     off += s_ex;
     if (ws) ws->eyt = reinterpret_cast<float*>(b + off);
     off += s_ey;
+    const size_t tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
+    if (ws) ws->colmask = reinterpret_cast<uint32_t*>(b + off);
+    off += align_up(sizeof(uint32_t) * tc * static_cast<size_t>(count), 256);
+    if (ws) ws->rowmask = reinterpret_cast<uint32_t*>(b + off);
+    off += align_up(sizeof(uint32_t) * tr * static_cast<size_t>(count), 256);
     return off;
 }
 
@@ -163,7 +169,6 @@ __device__ __forceinline__ int frame_points_warp(const double* __restrict__ w2c,
     if (lane == 0) {
         meta[f].n_valid = n_valid;
         meta[f].zmax_bits = 0u;
-        meta[f].xa = INT_MAX; meta[f].xb = -1; meta[f].ya = INT_MAX; meta[f].yb = -1;
     }
     if (lane == pp.n_points - 1) {                      // the frame's own point (i == t)
         int index = -1;
@@ -363,91 +368,40 @@ __device__ __forceinline__ float eval_tile(const float* __restrict__ exf, const 
 
 __global__ void __launch_bounds__(256)
 norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const float* __restrict__ ex,
-            const float* __restrict__ eyt, int npad, int width, int height, int norm) {
+            const float* __restrict__ eyt, uint32_t* __restrict__ colmask, uint32_t* __restrict__ rowmask, int npad,
+            int width, int height, int norm) {
     extern __shared__ float sm_f[];
     __shared__ double s_dred[8];
-    pdl_wait();                             // tables_kernel's output
-    pdl_trigger();
-    const int f = blockIdx.y, part = blockIdx.x;
-    const int n_valid = meta[f].n_valid;
-    if (part != 0 && (norm != MF_NORM_MAX || n_valid == 0 || meta[f].pad != 0)) return;
-    const float* exf = ex + static_cast<size_t>(f) * npad * width;
-    const float* eyf = eyt + static_cast<size_t>(f) * height * npad;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (n_valid == 0 || meta[f].pad != 0) {
-        if (threadIdx.x == 0) meta[f].inv_z = 0.f;
-        return;
-    }
-    __shared__ int s_box[4];                // xa, xb, ya, yb of the frame's non-negligible region
-    if (threadIdx.x == 0) {
-        s_box[0] = INT_MAX; s_box[1] = -1; s_box[2] = INT_MAX; s_box[3] = -1;
-    }
-    __syncthreads();
-    if (norm != MF_NORM_MAX) {
-        // bounding box straight from the tables (these modes are not latency-critical)
-        int lo = INT_MAX, hi = -1;
-        for (int x = threadIdx.x; x < width; x += blockDim.x)
-            for (int j = 0; j < n_valid; ++j)
-                if (exf[static_cast<size_t>(j) * width + x] >= kCullBelow) { lo = min(lo, x); hi = max(hi, x); }
-        if (hi >= 0) { atomicMin(&s_box[0], lo); atomicMax(&s_box[1], hi); }
-        lo = INT_MAX; hi = -1;
-        for (int y = threadIdx.x; y < height; y += blockDim.x)
-            for (int j = 0; j < n_valid; ++j)
-                if (eyf[static_cast<size_t>(y) * npad + j] >= kCullBelow) { lo = min(lo, y); hi = max(hi, y); }
-        if (hi >= 0) { atomicMin(&s_box[2], lo); atomicMax(&s_box[3], hi); }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            meta[f].xa = s_box[0]; meta[f].xb = s_box[1]; meta[f].ya = s_box[2]; meta[f].yb = s_box[3];
-        }
-    }
-    if (norm == MF_NORM_NONE) {
-        if (threadIdx.x == 0) meta[f].inv_z = meta[f].out_scale;
-        return;
-    }
-    if (norm == MF_NORM_SUM) {
-        // sum_xy U' = sum_j (sum_x Ex_j)(sum_y Ey_j), closed form from the tables, fp64
-        double total = 0.0;
-        for (int j = 0; j < n_valid; ++j) {
-            double sx = 0.0, sy = 0.0;
-            for (int x = threadIdx.x; x < width; x += blockDim.x) sx += exf[static_cast<size_t>(j) * width + x];
-            for (int y = threadIdx.x; y < height; y += blockDim.x) sy += eyf[static_cast<size_t>(y) * npad + j];
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                sx += __shfl_xor_sync(0xffffffffu, sx, o);
-                sy += __shfl_xor_sync(0xffffffffu, sy, o);
-            }
-            __syncthreads();
-            if (lane == 0) s_dred[warp] = sx;
-            __syncthreads();
-            double bx = 0.0;
-            for (int w = 0; w < 8; ++w) bx += s_dred[w];
-            __syncthreads();
-            if (lane == 0) s_dred[warp] = sy;
-            __syncthreads();
-            double by = 0.0;
-            for (int w = 0; w < 8; ++w) by += s_dred[w];
-            total += bx * by;
-        }
-        if (threadIdx.x == 0) meta[f].inv_z = total > 0.0 ? static_cast<float>(1.0 / total) : 0.f;
-        return;
-    }
-    // ---- MF_NORM_MAX ----
-    // Exact branch and bound.  Every step issues all of its (independent) global loads before using any of them:
-    // the kernel is a chain of memory latencies, not of arithmetic.
-    const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
-    float* mx = sm_f;                       // [npad][tc] max over the tile's columns of Ex_j
-    float* my = sm_f + npad * tc;           // [npad][tr]
     __shared__ float4 s_pts[kMaxPoints];
     __shared__ unsigned s_best;             // bit pattern of a lower bound of the frame's maximum
     __shared__ unsigned s_exact;            // bit pattern of the largest exactly evaluated pixel of this CTA
     __shared__ int s_count;
     __shared__ int s_list[kMaxSurvivors];
-    if (threadIdx.x < kMaxPoints)
+    pdl_wait();                             // tables_kernel's output
+    pdl_trigger();
+    const int f = blockIdx.y, part = blockIdx.x;
+    const int n_valid = meta[f].n_valid;
+    const bool empty = n_valid == 0 || meta[f].pad != 0;
+    if (part != 0 && (norm != MF_NORM_MAX || empty)) return;
+    const float* exf = ex + static_cast<size_t>(f) * npad * width;
+    const float* eyf = eyt + static_cast<size_t>(f) * height * npad;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (empty) {                            // renders as zeros: render_kernel never reads the masks when the scale is 0
+        if (threadIdx.x == 0) meta[f].inv_z = 0.f;
+        return;
+    }
+    // Every step below issues all of its (independent) global loads before using any of them: the kernel is a chain
+    // of memory latencies, not of arithmetic.
+    const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
+    float* mx = sm_f;                       // [npad][tc] largest Ex_j over the tile's columns (Ex_j is unimodal)
+    float* my = sm_f + npad * tc;           // [npad][tr]
+    float* centre = my + npad * tr;         // [kMaxPoints] map value at each centre's pixel
+    float* tile_buf = centre + kMaxPoints;  // [8 warps][kTile rows][kMaxPoints] staged row factors
+    if (threadIdx.x < kMaxPoints) {
         s_pts[threadIdx.x] = threadIdx.x < n_valid ? pts[static_cast<size_t>(f) * kMaxPoints + threadIdx.x]
                                                    : make_float4(0.f, 0.f, 1.f, 0.f);
-    float* centre = sm_f + npad * (tc + tr);                    // [kMaxPoints] map value at each centre's pixel
-    float* tile_buf = centre + kMaxPoints;                      // [8 warps][kTile rows][kMaxPoints] staged row factors
-    if (threadIdx.x < kMaxPoints) centre[threadIdx.x] = 0.f;
+        centre[threadIdx.x] = 0.f;
+    }
     if (threadIdx.x == 0) {
         s_best = 0u;
         s_exact = 0u;
@@ -491,41 +445,71 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
             if (i < npad * tr) my[i] = val[u];
         }
     }
-    // lower bound: the map at the pixel nearest to each centre; one (centre p, term k) product per thread, summed over k
-    // in any order (a bound, not the result: the tile holding that pixel is evaluated exactly below)
-    for (int base = 0; base < n_valid * npad; base += 256) {
-        const int i = base + threadIdx.x;
-        float term = 0.f;
-        if (i < n_valid * npad) {
-            const int p = i / npad, k = i - p * npad;
-            const int x = clamp_round(s_pts[p].x, 0, width - 1), y = clamp_round(s_pts[p].y, 0, height - 1);
-            term = __ldg(exf + static_cast<size_t>(k) * width + x) * __ldg(eyf + static_cast<size_t>(y) * npad + k);
+    if (norm == MF_NORM_MAX) {
+        // lower bound: the map at the pixel nearest to each centre; one (centre p, term k) product per thread, summed
+        // over k in any order (a bound, not the result: the tile holding that pixel is evaluated exactly below)
+        for (int base = 0; base < n_valid * npad; base += 256) {
+            const int i = base + threadIdx.x;
+            float term = 0.f;
+            if (i < n_valid * npad) {
+                const int p = i / npad, k = i - p * npad;
+                const int x = clamp_round(s_pts[p].x, 0, width - 1), y = clamp_round(s_pts[p].y, 0, height - 1);
+                term = __ldg(exf + static_cast<size_t>(k) * width + x) * __ldg(eyf + static_cast<size_t>(y) * npad + k);
+            }
+            // npad is 8, 16, 24 or 32: groups of 8 lanes never straddle two centres
+            term += __shfl_xor_sync(0xffffffffu, term, 1);
+            term += __shfl_xor_sync(0xffffffffu, term, 2);
+            term += __shfl_xor_sync(0xffffffffu, term, 4);
+            if ((lane & 7) == 0 && i < n_valid * npad) atomicAdd(&centre[i / npad], term);
         }
-        // npad is 8, 16, 24 or 32: groups of 8 lanes never straddle two centres
-        term += __shfl_xor_sync(0xffffffffu, term, 1);
-        term += __shfl_xor_sync(0xffffffffu, term, 2);
-        term += __shfl_xor_sync(0xffffffffu, term, 4);
-        if ((lane & 7) == 0 && i < n_valid * npad) atomicAdd(&centre[i / npad], term);
     }
     __syncthreads();
-    if (threadIdx.x < n_valid) atomicMax(&s_best, __float_as_uint(fmaxf(centre[threadIdx.x], 0.f) * 0.9999f));
     if (part == 0) {
-        // bounding box at tile granularity: mx / my hold each point's largest factor per tile column / row
+        // which points matter in which 32-pixel column / row strip: render_kernel skips the others (and writes exact
+        // zeros where none matters).  A factor below kCullBelow adds less than that fraction of the map's peak.
         for (int i = threadIdx.x; i < tc + tr; i += blockDim.x) {
             const bool col = i < tc;
             const int t = col ? i : i - tc;
-            bool any = false;
-            for (int j = 0; j < n_valid; ++j) any |= (col ? mx[j * tc + t] : my[j * tr + t]) >= kCullBelow;
-            if (any) {
-                atomicMin(&s_box[col ? 0 : 2], t * kTile);
-                atomicMax(&s_box[col ? 1 : 3], min(t * kTile + kTile, col ? width : height) - 1);
-            }
+            uint32_t m = 0u;
+            for (int j = 0; j < n_valid; ++j)
+                if ((col ? mx[j * tc + t] : my[j * tr + t]) >= kCullBelow) m |= 1u << j;
+            (col ? colmask + static_cast<size_t>(f) * tc : rowmask + static_cast<size_t>(f) * tr)[t] = m;
         }
     }
-    __syncthreads();
-    if (part == 0 && threadIdx.x == 0) {
-        meta[f].xa = s_box[0]; meta[f].xb = s_box[1]; meta[f].ya = s_box[2]; meta[f].yb = s_box[3];
+    if (norm == MF_NORM_NONE) {
+        if (threadIdx.x == 0) meta[f].inv_z = meta[f].out_scale;
+        return;
     }
+    if (norm == MF_NORM_SUM) {
+        // sum_xy U' = sum_j (sum_x Ex_j)(sum_y Ey_j), closed form from the tables, fp64
+        double total = 0.0;
+        for (int j = 0; j < n_valid; ++j) {
+            double sx = 0.0, sy = 0.0;
+            for (int x = threadIdx.x; x < width; x += blockDim.x) sx += exf[static_cast<size_t>(j) * width + x];
+            for (int y = threadIdx.x; y < height; y += blockDim.x) sy += eyf[static_cast<size_t>(y) * npad + j];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                sx += __shfl_xor_sync(0xffffffffu, sx, o);
+                sy += __shfl_xor_sync(0xffffffffu, sy, o);
+            }
+            __syncthreads();
+            if (lane == 0) s_dred[warp] = sx;
+            __syncthreads();
+            double bx = 0.0;
+            for (int w = 0; w < 8; ++w) bx += s_dred[w];
+            __syncthreads();
+            if (lane == 0) s_dred[warp] = sy;
+            __syncthreads();
+            double by = 0.0;
+            for (int w = 0; w < 8; ++w) by += s_dred[w];
+            total += bx * by;
+        }
+        if (threadIdx.x == 0) meta[f].inv_z = total > 0.0 ? static_cast<float>(1.0 / total) : 0.f;
+        return;
+    }
+    // ---- MF_NORM_MAX: exact branch and bound ----
+    if (threadIdx.x < n_valid) atomicMax(&s_best, __float_as_uint(fmaxf(centre[threadIdx.x], 0.f) * 0.9999f));
+    __syncthreads();
     const float best = __uint_as_float(s_best);
     float exact = 0.f;
     // tile t belongs to warp (t mod 8*kNormBlocks) of the frame: neighbouring (surviving) tiles go to different warps
@@ -546,15 +530,13 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
     const int n_surv = s_count;
     if (n_surv > kMaxSurvivors) {
         // more survivors than the list holds (huge sigma): fall back to this CTA's whole share of the tiles
-        for (int i = warp; i * kNormBlocks + part < n_tiles; i += 8) {
+        for (int i = warp; i * kNormBlocks + part < n_tiles; i += 8)
             exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
                                                     i * kNormBlocks + part, tc, lane)));
-        }
     } else {
-        for (int i = warp; i < n_surv; i += 8) {
+        for (int i = warp; i < n_surv; i += 8)
             exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
                                                     s_list[i], tc, lane)));
-        }
     }
     // only exactly evaluated pixels may set Z (the bound above is 0.9999 x an approximately summed value); the tile
     // holding the true maximum always survives: its bound is >= the map's value there >= every centre value >= best
@@ -582,6 +564,7 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
 #define MF_RENDER_MINB 1
 #endif
 constexpr int kRowsPerThread = MF_RENDER_ROWS;
+constexpr int kStageRows = 2 * MF_RENDER_ROWS;   // row factors staged per warp in render_kernel
 constexpr int kRenderThreads = MF_RENDER_THREADS;
 
 __device__ __forceinline__ float4 ld_stream(const float4* p) {
@@ -623,6 +606,7 @@ __device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth
 template <int NP, bool HAS_DEPTH, bool HAS_G>
 __global__ void __launch_bounds__(kRenderThreads, MF_RENDER_MINB)
 render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const FrameMeta* __restrict__ meta,
+              const uint32_t* __restrict__ colmask, const uint32_t* __restrict__ rowmask,
               const float* __restrict__ depth, float* __restrict__ focus_map, float* __restrict__ guided,
               int width, int height, int blocks_per_frame, int norm) {
     pdl_wait();                             // norm_kernel's (and, through it, tables_kernel's) output
@@ -643,28 +627,44 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
     }
     const size_t img = static_cast<size_t>(f) * height * width + x;
 
-    // Outside columns [xa,xb] x rows [ya,yb] every term of Eq. 7 is below kCullBelow of the map's peak (S8(c)-D3):
-    // those pixels are written as exact zeros by a pure streaming loop.  The test is warp-uniform.
-    const bool cols_hit = x + 3 >= fm.xa && x <= fm.xb && y1 > y0;
-    const bool warp_live = __any_sync(0xffffffffu, cols_hit) && scale != 0.f;
-    const int ya = warp_live ? min(max(fm.ya, y0), y1) : y1;     // live rows of this thread: [ya, yb)
-    const int yb = warp_live ? min(max(fm.yb + 1, ya), y1) : y1;
+    // Which points matter for this warp's columns and this thread's 32-row strip (norm_kernel's strip masks): a point
+    // whose factor is below kCullBelow over the whole strip adds < 1e-13 of the map's peak (S8(c)-D3 allows 1e-12).
+    // Where no point matters the pixels are exact zeros, written by a pure streaming loop.  All tests are warp-uniform
+    // except the row strip, which differs only between lanes of a warp that straddles two strips.
+    static_assert(kRowsPerThread == kTile, "render_kernel's row strips are norm_kernel's tiles");
+    const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
+    uint32_t pts_live = 0u;
+    if (scale != 0.f && y1 > y0)
+        pts_live = (__ldg(colmask + static_cast<size_t>(f) * tc + (x >> 5)) | __ldg(colmask + static_cast<size_t>(f) * tc + ((x + 3) >> 5))) &
+                   __ldg(rowmask + static_cast<size_t>(f) * tr + rb);
+    pts_live = __reduce_or_sync(0xffffffffu, pts_live);
+    const int ya = pts_live ? y0 : y1, yb = y1;                  // rows computed by this thread: [ya, yb)
     stream_zero_rows<HAS_DEPTH, HAS_G>(depth, focus_map, guided, img, width, y0, ya);
-    if (__any_sync(0xffffffffu, ya < yb)) {
+    if (pts_live) {
         float4 e[NP];
         const float* exf = ex + static_cast<size_t>(f) * NP * width + x;
+        unsigned live = 0u;                 // groups of 4 points
 #pragma unroll
-        for (int j = 0; j < NP; ++j) e[j] = __ldg(reinterpret_cast<const float4*>(exf + static_cast<size_t>(j) * width));
-        // groups of 4 points whose column factors are negligible over all of this warp's columns are skipped
-        unsigned live = 0u;
+        for (int q = 0; q < NP / 4; ++q)
+            if (pts_live & (0xFu << (4 * q))) live |= 1u << q;
 #pragma unroll
-        for (int q = 0; q < NP / 4; ++q) {
-            float m = 0.f;
-#pragma unroll
-            for (int k = 4 * q; k < 4 * q + 4; ++k) m = fmaxf(m, fmaxf(fmaxf(e[k].x, e[k].y), fmaxf(e[k].z, e[k].w)));
-            if (__any_sync(0xffffffffu, m >= kCullBelow && ya < yb)) live |= 1u << q;
-        }
+        for (int j = 0; j < NP; ++j)
+            e[j] = (live & (1u << (j / 4))) ? __ldg(reinterpret_cast<const float4*>(exf + static_cast<size_t>(j) * width))
+                                            : make_float4(0.f, 0.f, 0.f, 0.f);
         const float4* eyrow = reinterpret_cast<const float4*>(eyt + static_cast<size_t>(f) * height * NP);
+        // The row factors of the warp's rows (one 32-row strip, two when the warp straddles strips) are staged in
+        // shared memory with one batch of coalesced loads, so the row loop below never waits on L2 for them.
+        extern __shared__ float s_rows[];                       // [warps][kStageRows][NP]
+        float* wbuf = s_rows + (threadIdx.x >> 5) * (kStageRows * NP);
+        const int ylo = __reduce_min_sync(0xffffffffu, ya < yb ? ya : INT_MAX);
+        const int yhi = __reduce_max_sync(0xffffffffu, ya < yb ? yb : 0);
+        const bool staged = yhi - ylo <= kStageRows;            // false only for images narrower than 128 pixels
+        if (staged) {
+            const int n4 = (yhi - ylo) * (NP / 4);
+            for (int i = threadIdx.x & 31; i < n4; i += 32)
+                reinterpret_cast<float4*>(wbuf)[i] = __ldg(eyrow + static_cast<size_t>(ylo) * (NP / 4) + i);
+            __syncwarp();
+        }
         constexpr int U = MF_RENDER_U;
         for (int y = ya; y < yb; y += U) {
             float4 d[U];
@@ -680,7 +680,8 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
 #pragma unroll
                     for (int q = 0; q < NP / 4; ++q) {
                         if (!(live & (1u << q))) continue;
-                        const float4 w = __ldg(eyrow + static_cast<size_t>(y + r) * (NP / 4) + q);
+                        const float4 w = staged ? reinterpret_cast<const float4*>(wbuf)[(y + r - ylo) * (NP / 4) + q]
+                                                : __ldg(eyrow + static_cast<size_t>(y + r) * (NP / 4) + q);
                         const float wy[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
@@ -700,7 +701,6 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
             }
         }
     }
-    stream_zero_rows<HAS_DEPTH, HAS_G>(depth, focus_map, guided, img, width, yb, y1);
 }
 
 template <int NP>
@@ -710,12 +710,17 @@ static void launch_render(const Workspace& ws, const float* depth, float* focus_
     const long long threads = static_cast<long long>(width / 4) * row_blocks;
     const int bpf = static_cast<int>((threads + kRenderThreads - 1) / kRenderThreads);
     const unsigned grid = static_cast<unsigned>(bpf) * static_cast<unsigned>(count);
+    const size_t smem = sizeof(float) * (kRenderThreads / 32) * kStageRows * NP;
+    if (smem > 48 * 1024) {
+        cudaFuncSetAttribute(render_kernel<NP, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        cudaFuncSetAttribute(render_kernel<NP, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    }
     if (guided)
-        launch_pdl(render_kernel<NP, true, true>, dim3(grid), dim3(kRenderThreads), 0, stream, ws.ex, ws.eyt, ws.meta, depth,
-                   focus_map, guided, width, height, bpf, norm);
+        launch_pdl(render_kernel<NP, true, true>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
+                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm);
     else
-        launch_pdl(render_kernel<NP, false, false>, dim3(grid), dim3(kRenderThreads), 0, stream, ws.ex, ws.eyt, ws.meta,
-                   depth, focus_map, guided, width, height, bpf, norm);
+        launch_pdl(render_kernel<NP, false, false>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
+                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm);
 }
 
 }  // namespace mf
@@ -795,7 +800,8 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         return launch_pdl(norm_kernel, dim3(kNormBlocks, n), dim3(256), smem, q, ws.pts + static_cast<size_t>(f0) * kMaxPoints,
-                          ws.meta + f0, ex, eyt, npad, width, height, static_cast<int>(params->norm));
+                          ws.meta + f0, ex, eyt, ws.colmask + static_cast<size_t>(f0) * tc, ws.rowmask + static_cast<size_t>(f0) * tr,
+                          npad, width, height, static_cast<int>(params->norm));
     };
     // the HBM-bound pass over frames [f0, f0+n)
     auto render = [&](int f0, int n, cudaStream_t q) -> cudaError_t {
@@ -803,6 +809,8 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
         w.meta = ws.meta + f0;
         w.ex = ws.ex + static_cast<size_t>(f0) * npad * width;
         w.eyt = ws.eyt + static_cast<size_t>(f0) * height * npad;
+        w.colmask = ws.colmask + static_cast<size_t>(f0) * tc;
+        w.rowmask = ws.rowmask + static_cast<size_t>(f0) * tr;
         const float* d = depth ? depth + f0 * img : nullptr;
         float* m = focus_map + f0 * img;
         float* gd = guided_depth ? guided_depth + f0 * img : nullptr;

@@ -118,6 +118,38 @@ def test_suburban_window_sampled_rows(api):
     _check(api, 2, w, p, 16, oa.FRAME, synth.seed_for(1, 0), rows=rows, lse=True)
 
 
+def _a7_rows(w, p, seed, n_random=256, edge=64):
+    """Reading A7: seeded random rows + the first and last rows + the rows next to every frame boundary."""
+    rng = np.random.default_rng(seed)
+    s_len = w * p
+    return np.unique(np.concatenate([np.arange(edge), np.arange(s_len - edge, s_len), rng.integers(0, s_len, n_random),
+                                     np.concatenate([[f * p - 1, f * p] for f in range(1, w)])]))
+
+
+@pytest.mark.parametrize("cfg_idx,windows,check", [
+    (2, 2, [1]),          # city:   W=16, S=12432
+    (3, 4, [0, 3]),       # campus: W=32, S=24864, 4 windows per launch = the launch configuration bench.py times
+    (4, 1, [0]),          # town:   W=64, S=49728
+])
+def test_full_size_configs_sampled_rows(api, cfg_idx, windows, check):
+    # BASELINE.json configs[2..4] at full size: the oracle evaluates sampled query rows exactly (reading A7)
+    cfg = synth.CONFIGS[cfg_idx]
+    w, p, heads = cfg["W"], cfg["P"], cfg["H"]
+    q, k, v = synth.qkv(windows, w * p, heads, 64, synth.seed_for(cfg_idx, 0), device="cuda")
+    rows = _a7_rows(w, p, 11 + cfg_idx)
+    for mode in (oa.GLOBAL, oa.FRAME):
+        out, lse = api.window_attention(q, k, v, w, p, mode, return_lse=True)
+        torch.cuda.synchronize()
+        assert torch.isfinite(out.float()).all()
+        for n in check:
+            ref, lse_ref = oa.window_attention(_to64(q[n:n + 1]), _to64(k[n:n + 1]), _to64(v[n:n + 1]), w, p, mode, rows=rows)
+            d = _to64(out[n:n + 1, torch.from_numpy(rows).cuda()]) - ref
+            max_abs, rel = np.abs(d).max(), np.linalg.norm(d) / np.linalg.norm(ref)
+            assert max_abs <= MAX_ABS and rel <= REL_L2, (cfg_idx, mode, n, max_abs, rel)
+            g = lse[n:n + 1].cpu().numpy().astype(np.float64)[:, :, rows]
+            assert np.abs(g - lse_ref).max() <= 4e-3
+
+
 def test_errors(api):
     q, k, v = synth.qkv(1, 64, 1, 32, 1, device="cuda")
     with pytest.raises(api.MfError):
