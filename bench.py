@@ -46,6 +46,15 @@ def measured_peaks():
     return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, source="fallback")
 
 
+# DRAM traffic per GLOBAL attention launch from the committed ncu captures (profiles/r1_ncu_full_v3.md), keyed by
+# (config index, windows per launch).  Other launch shapes have no capture: null.
+NCU_TRAFFIC_BYTES = {(3, 1): 152.94e6 + 34.52e6, (3, 4): 612.33e6 + 187.98e6}
+
+
+def ncu_traffic(cfg_idx, windows_per_launch):
+    return NCU_TRAFFIC_BYTES.get((cfg_idx, windows_per_launch))
+
+
 class ClockSampler:
     """Polls nvidia-smi during the timed region (B200_PROFILING.md clocks line)."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -347,7 +356,10 @@ def main():
                 "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['source']}); kernel timed inside a long step",
                 "frac_of_burst": tflops / peaks["tf_burst"], "frac_of_nominal_2250": tflops / 2250.0,
                 "flops_per_launch": wl.flops_global * wl.B, "ms_per_launch": g_launch_ms,
-                "share_of_step": g_ms / ms_total, "traffic": None}
+                "share_of_step": g_ms / ms_total, "traffic": ncu_traffic(args.config, wl.B),
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this "
+                                  "launch shape (profiles/r1_ncu_full_v3.md); algorithmic Q,K,V,O bytes per launch = "
+                                  f"{8.0 * wl.S * wl.H * wl.D * wl.B:.0f}"}
     focus = {"bound": "hbm", "kernel": "mf_motion_focus (points+tables+norm+render, 12 B/pixel algorithmic)",
              "achieved": focus_gbs, "peak": peaks["hbm"], "unit": "GB/s", "frac": focus_gbs / peaks["hbm"],
              "share_of_step": f_ms / ms_total}
