@@ -123,7 +123,7 @@ class Workload:
         # algorithmic work
         self.flops_global = 4.0 * self.S * self.S * self.H * self.D                  # per window-layer
         self.flops_frame = 4.0 * self.W * self.P * self.P * self.H * self.D
-        self.n_global = self.layers // 2
+        self.n_global = self.layers // 2 if self.layers > 1 else 1      # tiny config: its one layer is GLOBAL (BJ configs[0])
         self.n_frame = self.layers - self.n_global
         self.flops_step = self.Nw * (self.n_global * self.flops_global + self.n_frame * self.flops_frame)
         self.focus_bytes_step = 12.0 * self.N * self.width * self.height
@@ -154,7 +154,7 @@ class Workload:
             b1 = min(b0 + self.B, self.Nw)
             qb, kb, vb = self.q[b0:b1], self.k[b0:b1], self.v[b0:b1]
             for layer in range(self.layers):
-                mode = api.ATTN_FRAME if layer % 2 == 0 else api.ATTN_GLOBAL          # reading A3
+                mode = api.ATTN_FRAME if (layer % 2 == 0 and self.layers > 1) else api.ATTN_GLOBAL   # reading A3
                 out = self.o[layer % 2][: b1 - b0]
                 if ev_global is not None and mode == api.ATTN_GLOBAL:
                     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -203,7 +203,8 @@ class Workload:
         api, c = self.api, self.cfg
         for b0 in range(0, self.Nw, self.B):
             nb = min(self.B, self.Nw - b0)
-            api.window_attention_host(self.hq[:nb], self.hk[:nb], self.hv[:nb], self.W, self.P, api.ATTN_FRAME,
+            api.window_attention_host(self.hq[:nb], self.hk[:nb], self.hv[:nb], self.W, self.P,
+                                      api.ATTN_FRAME if self.layers > 1 else api.ATTN_GLOBAL,
                                       out=self.ho[:nb], num_layers=self.layers)
         for f0 in range(0, self.N, self.chunk):
             f1 = min(f0 + self.chunk, self.N)
@@ -246,7 +247,7 @@ def oracle_sample(cfg_idx, wl_dims, rows=1024):
     t0 = time.perf_counter()
     orr.focus_map(frames[min(N - 1, 20)]["points"], cfg["width"], cfg["height"], orr.NORM_MAX, depth)
     t_render = time.perf_counter() - t0
-    n_global = layers // 2
+    n_global = layers // 2 if layers > 1 else 1
     n_frame = layers - n_global
     total = Nw * (n_global * t_global * S / rows + n_frame * t_frame * W) + t_pose + N * t_render
     cores = len(os.sched_getaffinity(0))
