@@ -157,6 +157,35 @@ mf_status mf_chain_and_focus_host(const float* local_w2c, int num_windows, int W
                                   double* global_w2c, float* focus_map, float* guided_depth,
                                   float* focus_uv, int32_t* focus_index, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Dense layers around the window attention.  PAPER.md treats the transformer as
+ * a black box; BJ fixes only "24-layer d=1024 H=16 stack".  The standard pre-norm block is
+ * taken as reading E1-E4: h = x + W_o Attn(W_qkv LN1(x)), y = h + W_2 GELU(W_1 LN2(h)).
+ *
+ * mf_linear:  out = act(x w^T + bias) (+ residual), bf16 operands, fp32 accumulation (tcgen05 MMA into
+ * TMEM), bf16 output rounded to nearest even.
+ *   x        bf16 [M, K] row-major              w     bf16 [N, K] row-major (nn.Linear layout)
+ *   bias     fp32 [N] or NULL                   residual  bf16 [M, N] or NULL (single output only)
+ *   out0..2  bf16 [M, n_split] each: output tensor i receives columns [i*n_split, (i+1)*n_split) of the
+ *            product, so N = 3*n_split writes q | k | v as three [tokens, heads*head_dim] tensors in one
+ *            pass; N = n_split writes one tensor (out1 = out2 = NULL).
+ *   act      MF_ACT_GELU is the exact erf form (reading E3).
+ * K % 64 == 0 and n_split % 256 == 0 are required (MF_ERR_UNSUPPORTED otherwise); all tensors 16-byte
+ * aligned; outputs must not alias x (residual may equal out0: each element is read before it is written
+ * by the same thread).
+ *
+ * mf_layernorm: out = (x - mean) / sqrt(var + eps) * gamma + beta over the last axis (biased variance,
+ * fp32 statistics), x/out bf16 [M, d], gamma/beta fp32 [d]; d in {256, 512, 768, 1024}.
+ */
+typedef enum { MF_ACT_NONE = 0, MF_ACT_GELU = 1 } mf_activation;
+
+mf_status mf_linear(const void* x, const void* w, const float* bias, const void* residual, void* out0,
+                    void* out1, void* out2, int M, int N, int K, int n_split, mf_activation act,
+                    void* stream);
+
+mf_status mf_layernorm(const void* x, const float* gamma, const float* beta, float eps, void* out, int M,
+                       int d, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

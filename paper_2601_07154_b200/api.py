@@ -15,10 +15,11 @@ VEC_ACCEL, VEC_VELOCITY = 0, 1
 MAG_RAW, MAG_UNIT = 0, 1
 NORM_MAX, NORM_SUM, NORM_NONE = 0, 1, 2
 PTS_CURRENT_FRAME, PTS_OWN_FRAME = 0, 1
+ACT_NONE, ACT_GELU = 0, 1
 
 EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
-           "mf_window_attention_host", "mf_chain_and_focus_host"]
+           "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm"]
 
 
 class MfError(RuntimeError):
@@ -61,6 +62,8 @@ def lib():
         L.mf_window_attention_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, vp]
         L.mf_chain_and_focus_host.argtypes = [vp, ci, ci, ci, ci, ci, Intrinsics, ci, ci, ci, ci, vp,
                                               ctypes.POINTER(FocusParams), vp, vp, vp, vp, vp, vp]
+        L.mf_linear.argtypes = [vp, vp, vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp]
+        L.mf_layernorm.argtypes = [vp, vp, vp, cf, vp, ci, ci, vp]
         _lib = L
     return _lib
 
@@ -208,3 +211,39 @@ def chain_and_focus_host(local_w2c, stride, num_frames, fx, fy, cx, cy, width, h
                                          _ptr(depth), ctypes.byref(params), _ptr(poses), _ptr(fmap), _ptr(guided),
                                          _ptr(uv), _ptr(idx), _stream()))
     return {"global_w2c": poses, "focus_map": fmap, "guided_depth": guided, "focus_uv": uv, "focus_index": idx}
+
+
+def linear(x, w, bias=None, residual=None, act=ACT_NONE, splits=1, out=None):
+    """out = act(x w^T + bias) (+ residual).  x bf16 [M,K], w bf16 [N,K]; `splits` = 1 or 3 output tensors
+    [M, N/splits] (3: q | k | v).  Returns a tensor (splits == 1) or a tuple of tensors."""
+    _dev(x, torch.bfloat16, "x")
+    _dev(w, torch.bfloat16, "w")
+    if x.dim() != 2 or w.dim() != 2 or x.shape[1] != w.shape[1]:
+        raise MfError("linear: x [M,K] and w [N,K] expected")
+    m, k = x.shape
+    n = w.shape[0]
+    if n % splits:
+        raise MfError("linear: N not divisible by splits")
+    if bias is not None:
+        _dev(bias, torch.float32, "bias")
+    if residual is not None:
+        _dev(residual, torch.bfloat16, "residual")
+    outs = list(out) if out is not None else [torch.empty((m, n // splits), device=x.device, dtype=torch.bfloat16)
+                                              for _ in range(splits)]
+    for o in outs:
+        _dev(o, torch.bfloat16, "out")
+    o3 = outs + [None] * (3 - len(outs))
+    _check(lib().mf_linear(_ptr(x), _ptr(w), _ptr(bias), _ptr(residual), _ptr(o3[0]), _ptr(o3[1]), _ptr(o3[2]), m, n, k,
+                           n // splits, act, _stream()))
+    return outs[0] if splits == 1 else tuple(outs)
+
+
+def layernorm(x, gamma, beta, eps=1e-6, out=None):
+    _dev(x, torch.bfloat16, "x")
+    _dev(gamma, torch.float32, "gamma")
+    _dev(beta, torch.float32, "beta")
+    if out is None:
+        out = torch.empty_like(x)
+    _dev(out, torch.bfloat16, "out")
+    _check(lib().mf_layernorm(_ptr(x), _ptr(gamma), _ptr(beta), float(eps), _ptr(out), x.shape[0], x.shape[1], _stream()))
+    return out

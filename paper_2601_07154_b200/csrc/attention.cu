@@ -21,6 +21,7 @@
 // [windows*W, P, H, D].
 #include "common.h"
 #include "sm100_ptx.cuh"
+#include "tensormap.h"
 
 #include <cuda_bf16.h>
 
@@ -372,22 +373,6 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 // Host side: tensor maps + launch
 // ------------------------------------------------------------------------------------------------
 namespace mf {
-
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn encode_fn() {
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
-    }
-    return fn;
-}
 
 // bf16 [sequences, seq_len, heads, 64] -> 4-D map (d, head, token, sequence), box = 64 x 1 x 128 x 1
 static mf_status make_map(CUtensorMap* map, const void* base, int sequences, int seq_len, int heads) {

@@ -1,0 +1,326 @@
+// mf_linear: out = act(x w^T + bias) (+ residual), bf16 in / fp32 accumulate / bf16 out, for sm_100a
+// (the QKV projection, output projection and MLP around the window attention; reading E1-E4).
+//
+// Persistent kernel, one CTA per SM, 192 threads:
+//   warp 0     TMA producer: x tile (128 rows x 64 k) and w tile (256 rows x 64 k), SWIZZLE_128B, 4-stage ring
+//   warp 1     tcgen05.mma issuer (one thread): D[128 x 256] += x_tile w_tile^T, 4 MMAs of K=16 per stage,
+//              accumulator in TMEM, two accumulators (2 x 256 columns) so the epilogue of tile i overlaps the
+//              main loop of tile i+1
+//   warps 2-5  epilogue: tcgen05.ld 32 columns at a time (TMEM lane = output row), + bias, GELU, + residual,
+//              round to bf16, 64 B per thread and chunk straight to global memory
+// Output tiles are visited n-fastest, so the CTAs running together share one band of x rows in L2 while w (a few
+// MB) stays L2-resident.  Columns may be split over up to three output tensors (q | k | v): n_split columns each.
+#include "common.h"
+#include "sm100_ptx.cuh"
+#include "tensormap.h"
+
+#include <cuda_bf16.h>
+
+namespace mf {
+
+constexpr int kGM = 128, kGN = 256, kGK = 64, kGStages = 4;
+constexpr int kGThreads = 192;
+constexpr int kATile = kGM * kGK * 2;      // 16 KB
+constexpr int kBTile = kGN * kGK * 2;      // 32 KB
+
+struct GemmSmem {
+    alignas(1024) uint8_t a[kGStages][kATile];
+    alignas(1024) uint8_t b[kGStages][kBTile];
+    alignas(8) uint64_t full[kGStages];
+    uint64_t empty[kGStages], acc_full[2], acc_empty[2];
+    uint32_t tmem_base;
+};
+
+struct GemmParams {
+    int M, N, K, n_split;
+    int m_tiles, n_tiles;
+    const float* bias;
+    const __nv_bfloat16* residual;
+    __nv_bfloat16* out[3];
+    int act;
+};
+
+constexpr uint32_t kIdescGemm = ptx::idesc_bf16_f32(kGM, kGN, 0, 0);
+
+__device__ __forceinline__ float gelu_erf(float t) { return 0.5f * t * (1.0f + erff(t * 0.70710678118654752f)); }
+
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 :: "r"(ptx::smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(ptx::smem_u32(bar)), "r"(c0), "r"(c1)
+                 : "memory");
+}
+
+__global__ void __launch_bounds__(kGThreads, 1)
+linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__ CUtensorMap map_w, const GemmParams prm) {
+    extern __shared__ uint8_t smem_raw[];
+    GemmSmem& sm = *reinterpret_cast<GemmSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_tiles_total = prm.m_tiles * prm.n_tiles;
+    const int k_steps = prm.K / kGK;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&map_x);
+        ptx::prefetch_tensormap(&map_w);
+        for (int s = 0; s < kGStages; ++s) {
+            ptx::mbar_init(&sm.full[s], 1);
+            ptx::mbar_init(&sm.empty[s], 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            ptx::mbar_init(&sm.acc_full[b], 1);
+            ptx::mbar_init(&sm.acc_empty[b], 4);           // one arrival per epilogue warp
+        }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 1) ptx::tmem_alloc(&sm.tmem_base, 512);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            int it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x) {
+                const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
+                for (int ks = 0; ks < k_steps; ++ks, ++it) {
+                    const int st = it % kGStages;
+                    ptx::mbar_wait(&sm.empty[st], ((it / kGStages) & 1) ^ 1);
+                    ptx::mbar_arrive_expect_tx(&sm.full[st], kATile + kBTile);
+                    tma_load_2d(sm.a[st], &map_x, &sm.full[st], ks * kGK, mt * kGM);
+                    tma_load_2d(sm.b[st], &map_w, &sm.full[st], ks * kGK, nt * kGN);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            int it = 0, local = 0;
+            for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x, ++local) {
+                const int buf = local & 1;
+                ptx::mbar_wait(&sm.acc_empty[buf], ((local >> 1) & 1) ^ 1);     // epilogue has drained this accumulator
+                ptx::tc_fence_after();
+                const uint32_t d = tmem + buf * kGN;
+                for (int ks = 0; ks < k_steps; ++ks, ++it) {
+                    const int st = it % kGStages;
+                    ptx::mbar_wait(&sm.full[st], (it / kGStages) & 1);
+                    ptx::tc_fence_after();
+                    const uint64_t ad = ptx::smem_desc_sw128(ptx::smem_u32(sm.a[st]));
+                    const uint64_t bd = ptx::smem_desc_sw128(ptx::smem_u32(sm.b[st]));
+#pragma unroll
+                    for (int i = 0; i < kGK / 16; ++i) ptx::mma_ss(d, ad + 2 * i, bd + 2 * i, kIdescGemm, (ks > 0 || i > 0) ? 1u : 0u);
+                    ptx::mma_commit(&sm.empty[st]);
+                }
+                ptx::mma_commit(&sm.acc_full[buf]);
+            }
+        }
+    } else {
+        // ===================== epilogue warps =====================
+        const int quarter = warp & 3;                      // TMEM lanes 32*quarter .. +31
+        const uint32_t lane_addr = static_cast<uint32_t>(quarter * 32) << 16;
+        int local = 0;
+        for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x, ++local) {
+            const int buf = local & 1;
+            const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
+            const int row = mt * kGM + quarter * 32 + lane;
+            const int n0 = nt * kGN;
+            const int which = n0 / prm.n_split, c0 = n0 - which * prm.n_split;
+            __nv_bfloat16* dst = prm.out[which] + static_cast<size_t>(row) * prm.n_split + c0;
+            const __nv_bfloat16* res = prm.residual ? prm.residual + static_cast<size_t>(row) * prm.N + n0 : nullptr;
+            ptx::mbar_wait(&sm.acc_full[buf], (local >> 1) & 1);
+            ptx::tc_fence_after();
+#pragma unroll 1
+            for (int c = 0; c < kGN / 32; ++c) {
+                uint32_t acc[32];
+                ptx::tmem_ld32(tmem + lane_addr + buf * kGN + 32 * c, acc);
+                ptx::tc_wait_ld();
+                if (row < prm.M) {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        float vals[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) vals[i] = __uint_as_float(acc[8 * g + i]);
+                        if (prm.bias) {
+                            const float4 b0 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 32 * c + 8 * g));
+                            const float4 b1 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 32 * c + 8 * g + 4));
+                            vals[0] += b0.x; vals[1] += b0.y; vals[2] += b0.z; vals[3] += b0.w;
+                            vals[4] += b1.x; vals[5] += b1.y; vals[6] += b1.z; vals[7] += b1.w;
+                        }
+                        if (prm.act == MF_ACT_GELU) {
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) vals[i] = gelu_erf(vals[i]);
+                        }
+                        if (res) {
+                            const uint4 r = __ldg(reinterpret_cast<const uint4*>(res + 32 * c + 8 * g));
+                            const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                vals[2 * i] += __uint_as_float(rr[i] << 16);
+                                vals[2 * i + 1] += __uint_as_float(rr[i] & 0xffff0000u);
+                            }
+                        }
+                        uint4 o;
+                        o.x = ptx::pack_bf16(vals[0], vals[1]);
+                        o.y = ptx::pack_bf16(vals[2], vals[3]);
+                        o.z = ptx::pack_bf16(vals[4], vals[5]);
+                        o.w = ptx::pack_bf16(vals[6], vals[7]);
+                        *reinterpret_cast<uint4*>(dst + 32 * c + 8 * g) = o;
+                    }
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&sm.acc_empty[buf]);
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+}  // namespace mf
+
+// ------------------------------------------------------------------------------------------------
+// LayerNorm (reading E4): one warp per row, bf16 in/out, fp32 statistics (two-pass over registers)
+// ------------------------------------------------------------------------------------------------
+namespace mf {
+
+template <int VEC>      // d = 32 * 8 * VEC channels: each lane holds VEC 16-byte chunks
+__global__ void __launch_bounds__(256)
+layernorm_kernel(const __nv_bfloat16* __restrict__ x, const float* __restrict__ gamma, const float* __restrict__ beta,
+                 float eps, __nv_bfloat16* __restrict__ out, int M) {
+    const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (row >= M) return;
+    constexpr int d = 32 * 8 * VEC;
+    const uint4* src = reinterpret_cast<const uint4*>(x + static_cast<size_t>(row) * d);
+    float v[8 * VEC];
+    float sum = 0.f;
+#pragma unroll
+    for (int c = 0; c < VEC; ++c) {
+        const uint4 u = __ldg(src + c * 32 + lane);
+        const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            v[8 * c + 2 * i] = __uint_as_float(w[i] << 16);
+            v[8 * c + 2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+            sum += v[8 * c + 2 * i] + v[8 * c + 2 * i + 1];
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const float mean = sum * (1.0f / d);
+    float sq = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8 * VEC; ++i) {
+        v[i] -= mean;
+        sq = fmaf(v[i], v[i], sq);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+    const float rstd = rsqrtf(sq * (1.0f / d) + eps);
+    uint4* dst = reinterpret_cast<uint4*>(out + static_cast<size_t>(row) * d);
+#pragma unroll
+    for (int c = 0; c < VEC; ++c) {
+        const int ch = (c * 32 + lane) * 8;
+        const float4 g0 = __ldg(reinterpret_cast<const float4*>(gamma + ch)), g1 = __ldg(reinterpret_cast<const float4*>(gamma + ch + 4));
+        const float4 b0 = __ldg(reinterpret_cast<const float4*>(beta + ch)), b1 = __ldg(reinterpret_cast<const float4*>(beta + ch + 4));
+        const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+        const float b[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+        float y[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) y[i] = fmaf(v[8 * c + i] * rstd, g[i], b[i]);
+        uint4 o;
+        o.x = ptx::pack_bf16(y[0], y[1]);
+        o.y = ptx::pack_bf16(y[2], y[3]);
+        o.z = ptx::pack_bf16(y[4], y[5]);
+        o.w = ptx::pack_bf16(y[6], y[7]);
+        dst[c * 32 + lane] = o;
+    }
+}
+
+// bf16 [rows, K] row-major -> 2-D map (k, row), box = 64 x box_rows, SWIZZLE_128B, zero OOB fill
+static mf_status make_map_2d(CUtensorMap* map, const void* base, long long rows, int K, int box_rows) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return fail(MF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+    cuuint64_t dims[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(rows)};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(K) * 2};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(kGK), static_cast<cuuint32_t>(box_rows)};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(MF_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", static_cast<int>(r));
+    return MF_OK;
+}
+
+}  // namespace mf
+
+extern "C" mf_status mf_linear(const void* x, const void* w, const float* bias, const void* residual, void* out0,
+                               void* out1, void* out2, int M, int N, int K, int n_split, mf_activation act,
+                               void* stream) {
+    using namespace mf;
+    if (!x || !w || !out0) return fail(MF_ERR_INVALID_ARG, "mf_linear: NULL tensor");
+    if (M < 1 || N < 1 || K < 1 || n_split < 1) return fail(MF_ERR_INVALID_ARG, "mf_linear: non-positive dimension");
+    if (act != MF_ACT_NONE && act != MF_ACT_GELU) return fail(MF_ERR_INVALID_ARG, "mf_linear: bad activation %d", static_cast<int>(act));
+    if (N % n_split != 0 || N / n_split > 3) return fail(MF_ERR_INVALID_ARG, "mf_linear: N must be 1..3 x n_split");
+    const int parts = N / n_split;
+    if ((parts > 1 && !out1) || (parts > 2 && !out2)) return fail(MF_ERR_INVALID_ARG, "mf_linear: missing output tensor");
+    if (residual && parts != 1) return fail(MF_ERR_INVALID_ARG, "mf_linear: residual needs a single output");
+    if (K % kGK != 0 || n_split % kGN != 0)
+        return fail(MF_ERR_UNSUPPORTED, "mf_linear: K %% 64 == 0 and n_split %% 256 == 0 required (K=%d, n_split=%d)", K, n_split);
+    if (!aligned16(x) || !aligned16(w) || !aligned16(out0) || (out1 && !aligned16(out1)) || (out2 && !aligned16(out2)) ||
+        (bias && !aligned16(bias)) || (residual && !aligned16(residual)))
+        return fail(MF_ERR_ALIGNMENT, "mf_linear: tensors must be 16-byte aligned");
+    if (out0 == x || out1 == x || out2 == x) return fail(MF_ERR_INVALID_ARG, "mf_linear: output aliases x");
+    mf_status st = require_sm100();
+    if (st != MF_OK) return st;
+    CUtensorMap mx, mw;
+    if ((st = make_map_2d(&mx, x, M, K, kGM)) != MF_OK) return st;
+    if ((st = make_map_2d(&mw, w, N, K, kGN)) != MF_OK) return st;
+    GemmParams prm;
+    prm.M = M; prm.N = N; prm.K = K; prm.n_split = n_split;
+    prm.m_tiles = (M + kGM - 1) / kGM;
+    prm.n_tiles = N / kGN;
+    prm.bias = bias;
+    prm.residual = static_cast<const __nv_bfloat16*>(residual);
+    prm.out[0] = static_cast<__nv_bfloat16*>(out0);
+    prm.out[1] = static_cast<__nv_bfloat16*>(out1);
+    prm.out[2] = static_cast<__nv_bfloat16*>(out2);
+    prm.act = act;
+    const long long tiles = static_cast<long long>(prm.m_tiles) * prm.n_tiles;
+    if (tiles > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_linear: too many tiles");
+    const int grid = static_cast<int>(tiles < sm_count() ? tiles : sm_count());
+    const int smem = static_cast<int>(sizeof(GemmSmem)) + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        MF_CUDA_OK(cudaFuncSetAttribute(linear_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    linear_kernel<<<grid, kGThreads, smem, static_cast<cudaStream_t>(stream)>>>(mx, mw, prm);
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}
+
+extern "C" mf_status mf_layernorm(const void* x, const float* gamma, const float* beta, float eps, void* out, int M,
+                                  int d, void* stream) {
+    using namespace mf;
+    if (!x || !gamma || !beta || !out) return fail(MF_ERR_INVALID_ARG, "mf_layernorm: NULL tensor");
+    if (M < 1 || d < 1 || !(eps >= 0.f)) return fail(MF_ERR_INVALID_ARG, "mf_layernorm: bad dimension or eps");
+    if (!aligned16(x) || !aligned16(out) || !aligned16(gamma) || !aligned16(beta))
+        return fail(MF_ERR_ALIGNMENT, "mf_layernorm: tensors must be 16-byte aligned");
+    mf_status st = require_sm100();
+    if (st != MF_OK) return st;
+    const unsigned grid = static_cast<unsigned>((static_cast<long long>(M) * 32 + 255) / 256);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const __nv_bfloat16* xi = static_cast<const __nv_bfloat16*>(x);
+    __nv_bfloat16* xo = static_cast<__nv_bfloat16*>(out);
+    switch (d) {
+        case 256: layernorm_kernel<1><<<grid, 256, 0, s>>>(xi, gamma, beta, eps, xo, M); break;
+        case 512: layernorm_kernel<2><<<grid, 256, 0, s>>>(xi, gamma, beta, eps, xo, M); break;
+        case 768: layernorm_kernel<3><<<grid, 256, 0, s>>>(xi, gamma, beta, eps, xo, M); break;
+        case 1024: layernorm_kernel<4><<<grid, 256, 0, s>>>(xi, gamma, beta, eps, xo, M); break;
+        default: return fail(MF_ERR_UNSUPPORTED, "mf_layernorm: d=%d (256, 512, 768, 1024 are built)", d);
+    }
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}

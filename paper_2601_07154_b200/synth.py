@@ -130,3 +130,21 @@ def depth(frames, height, width, seed, device="cpu"):
     g.manual_seed(seed)
     return torch.rand((frames, height, width), generator=g, device=device,
                       dtype=torch.float32) * 29.0 + 1.0
+
+
+def tokens(m, d, seed, device="cpu"):
+    """Activations ~ N(0,1) rounded to bf16, [m, d]."""
+    import torch
+    g = torch.Generator(device=device).manual_seed(int(seed))
+    return torch.randn((m, d), generator=g, device=device, dtype=torch.float32).to(torch.bfloat16)
+
+
+def linear_inputs(m, n, k, seed, device="cpu"):
+    """Seeded synthetic dense layer: x ~ N(0,1) bf16 [m,k]; w ~ N(0, 1/k) bf16 [n,k] (so x w^T ~ N(0,1)); bias ~ N(0, 0.1) fp32 [n].
+    Stand-in for trained weights, which are not available."""
+    import torch
+    g = torch.Generator(device=device).manual_seed(int(seed))
+    x = torch.randn((m, k), generator=g, device=device, dtype=torch.float32).to(torch.bfloat16)
+    w = (torch.randn((n, k), generator=g, device=device, dtype=torch.float32) / (k ** 0.5)).to(torch.bfloat16)
+    b = 0.1 * torch.randn((n,), generator=g, device=device, dtype=torch.float32)
+    return x, w, b
