@@ -1,13 +1,13 @@
 // mf_linear: out = act(x w^T + bias) (+ residual), bf16 in / fp32 accumulate / bf16 out, for sm_100a
 // (the QKV projection, output projection and MLP around the window attention; reading E1-E4).
 //
-// Persistent kernel, one CTA per SM, 192 threads:
+// Persistent kernel, one CTA per SM, 320 threads:
 //   warp 0     TMA producer: x tile (128 rows x 64 k) and w tile (256 rows x 64 k), SWIZZLE_128B, 4-stage ring
 //   warp 1     tcgen05.mma issuer (one thread): D[128 x 256] += x_tile w_tile^T, 4 MMAs of K=16 per stage,
 //              accumulator in TMEM, two accumulators (2 x 256 columns) so the epilogue of tile i overlaps the
 //              main loop of tile i+1
-//   warps 2-5  epilogue: tcgen05.ld 32 columns at a time (TMEM lane = output row), + bias, GELU, + residual,
-//              round to bf16, 64 B per thread and chunk straight to global memory
+//   warps 2-9  epilogue: tcgen05.ld 32 columns at a time (TMEM lane = output row; two warps per lane quarter, half
+//              of the columns each), + bias, GELU, + residual, round to bf16, 64 B per thread and chunk to global
 // Output tiles are visited n-fastest, so the CTAs running together share one band of x rows in L2 while w (a few
 // MB) stays L2-resident.  Columns may be split over up to three output tensors (q | k | v): n_split columns each.
 #include "common.h"
@@ -19,13 +19,15 @@
 namespace mf {
 
 constexpr int kGM = 128, kGN = 256, kGK = 64, kGStages = 4;
-constexpr int kGThreads = 192;
+constexpr int kEpiWarps = 8;               // two per TMEM lane quarter: each takes half of the tile's 256 columns
+constexpr int kGThreads = (2 + kEpiWarps) * 32;
 constexpr int kATile = kGM * kGK * 2;      // 16 KB
 constexpr int kBTile = kGN * kGK * 2;      // 32 KB
 
 struct GemmSmem {
     alignas(1024) uint8_t a[kGStages][kATile];
     alignas(1024) uint8_t b[kGStages][kBTile];
+    alignas(16) uint8_t stage[kEpiWarps][32 * 128];      // per epilogue warp: 32 rows x 64 bf16, XOR-swizzled 16-byte chunks
     alignas(8) uint64_t full[kGStages];
     uint64_t empty[kGStages], acc_full[2], acc_empty[2];
     uint32_t tmem_base;
@@ -42,7 +44,20 @@ struct GemmParams {
 
 constexpr uint32_t kIdescGemm = ptx::idesc_bf16_f32(kGM, kGN, 0, 0);
 
-__device__ __forceinline__ float gelu_erf(float t) { return 0.5f * t * (1.0f + erff(t * 0.70710678118654752f)); }
+// Reading E3 (exact erf GELU).  erf by Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7, far below the bf16 output's 2^-9):
+// erf(x) = 1 - (a1 t + ... + a5 t^5) exp(-x^2), t = 1 / (1 + p x), x >= 0; odd in x.
+__device__ __forceinline__ float gelu_erf(float v) {
+    const float x = fabsf(v) * 0.70710678118654752f;
+    float t;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, x, 1.0f)));
+    float poly = fmaf(1.061405429f, t, -1.453152027f);
+    poly = fmaf(poly, t, 1.421413741f);
+    poly = fmaf(poly, t, -0.284496736f);
+    poly = fmaf(poly, t, 0.254829592f);
+    const float e = ptx::ex2(-x * x * 1.4426950408889634f);
+    const float erf_abs = fmaf(-poly * t, e, 1.0f);
+    return 0.5f * v * (1.0f + copysignf(erf_abs, v));
+}
 
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
@@ -67,7 +82,7 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(&sm.acc_full[b], 1);
-            ptx::mbar_init(&sm.acc_empty[b], 4);           // one arrival per epilogue warp
+            ptx::mbar_init(&sm.acc_empty[b], kEpiWarps);   // one arrival per epilogue warp
         }
         ptx::fence_barrier_init();
     }
@@ -116,61 +131,99 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         }
     } else {
         // ===================== epilogue warps =====================
+        // A thread owns one output row (TMEM lane) and 64 consecutive columns per pass.  Rows are 2-8 KB apart in
+        // global memory, so the 32 x 128 B block of a pass goes through a per-warp, XOR-swizzled staging buffer: global
+        // accesses are then 4 rows x 128 B per warp instruction (4 wavefronts instead of 32), for the stores and for
+        // the residual loads alike.
         const int quarter = warp & 3;                      // TMEM lanes 32*quarter .. +31
+        const int chalf = (warp - 2) >> 2;                 // columns [128*chalf, 128*chalf + 128) of the tile
         const uint32_t lane_addr = static_cast<uint32_t>(quarter * 32) << 16;
+        uint4* stage = reinterpret_cast<uint4*>(sm.stage[warp - 2]);      // [32 rows][8 chunks of 16 B]
+        const int crow = lane >> 3, cchunk = lane & 7;     // coalesced phase: this lane's row (of 4) and 16-byte chunk
         int local = 0;
         for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x, ++local) {
             const int buf = local & 1;
             const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
-            const int row = mt * kGM + quarter * 32 + lane;
-            const int n0 = nt * kGN;
+            const int row0 = mt * kGM + quarter * 32;      // first of this warp's 32 rows
+            const int n0 = nt * kGN + 128 * chalf;         // first of this warp's 128 columns
             const int which = n0 / prm.n_split, c0 = n0 - which * prm.n_split;
-            __nv_bfloat16* dst = prm.out[which] + static_cast<size_t>(row) * prm.n_split + c0;
-            const __nv_bfloat16* res = prm.residual ? prm.residual + static_cast<size_t>(row) * prm.N + n0 : nullptr;
+            __nv_bfloat16* dst = prm.out[which] + c0;
+            // residual of both passes, fetched (coalesced) before the accumulator is waited for
+            uint4 rres[2][8];
+            if (prm.residual) {
+#pragma unroll
+                for (int g = 0; g < 2; ++g)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = row0 + 4 * i + crow;
+                        rres[g][i] = r < prm.M ? __ldg(reinterpret_cast<const uint4*>(prm.residual + static_cast<size_t>(r) * prm.N +
+                                                                                      n0 + 64 * g + 8 * cchunk))
+                                               : make_uint4(0u, 0u, 0u, 0u);
+                    }
+            }
             ptx::mbar_wait(&sm.acc_full[buf], (local >> 1) & 1);
             ptx::tc_fence_after();
-#pragma unroll 1
-            for (int c = 0; c < kGN / 32; ++c) {
-                uint32_t acc[32];
-                ptx::tmem_ld32(tmem + lane_addr + buf * kGN + 32 * c, acc);
-                ptx::tc_wait_ld();
-                if (row < prm.M) {
 #pragma unroll
-                    for (int g = 0; g < 4; ++g) {
-                        float vals[8];
+            for (int g = 0; g < 2; ++g) {
+                uint32_t acc[2][32];
+                ptx::tmem_ld32(tmem + lane_addr + buf * kGN + 128 * chalf + 64 * g, acc[0]);
+                ptx::tmem_ld32(tmem + lane_addr + buf * kGN + 128 * chalf + 64 * g + 32, acc[1]);
+                uint4 myres[8];                            // this thread's own row of the residual (8 x 8 bf16)
+                if (prm.residual) {
+                    __syncwarp();
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) vals[i] = __uint_as_float(acc[8 * g + i]);
-                        if (prm.bias) {
-                            const float4 b0 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 32 * c + 8 * g));
-                            const float4 b1 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 32 * c + 8 * g + 4));
-                            vals[0] += b0.x; vals[1] += b0.y; vals[2] += b0.z; vals[3] += b0.w;
-                            vals[4] += b1.x; vals[5] += b1.y; vals[6] += b1.z; vals[7] += b1.w;
-                        }
-                        if (prm.act == MF_ACT_GELU) {
+                    for (int i = 0; i < 8; ++i) stage[(4 * i + crow) * 8 + (cchunk ^ ((4 * i + crow) & 7))] = rres[g][i];
+                    __syncwarp();
 #pragma unroll
-                            for (int i = 0; i < 8; ++i) vals[i] = gelu_erf(vals[i]);
-                        }
-                        if (res) {
-                            const uint4 r = __ldg(reinterpret_cast<const uint4*>(res + 32 * c + 8 * g));
-                            const uint32_t rr[4] = {r.x, r.y, r.z, r.w};
-#pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                vals[2 * i] += __uint_as_float(rr[i] << 16);
-                                vals[2 * i + 1] += __uint_as_float(rr[i] & 0xffff0000u);
-                            }
-                        }
-                        uint4 o;
-                        o.x = ptx::pack_bf16(vals[0], vals[1]);
-                        o.y = ptx::pack_bf16(vals[2], vals[3]);
-                        o.z = ptx::pack_bf16(vals[4], vals[5]);
-                        o.w = ptx::pack_bf16(vals[6], vals[7]);
-                        *reinterpret_cast<uint4*>(dst + 32 * c + 8 * g) = o;
-                    }
+                    for (int j = 0; j < 8; ++j) myres[j] = stage[lane * 8 + (j ^ (lane & 7))];
+                    __syncwarp();
                 }
+                ptx::tc_wait_ld();
+                if (g == 1) {                              // the accumulator is in registers: hand it back to the MMA issuer
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&sm.acc_empty[buf]);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {              // 8 columns per step
+                    float vals[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) vals[i] = __uint_as_float(acc[j >> 2][8 * (j & 3) + i]);
+                    if (prm.bias) {
+                        const float4 b0 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 64 * g + 8 * j));
+                        const float4 b1 = __ldg(reinterpret_cast<const float4*>(prm.bias + n0 + 64 * g + 8 * j + 4));
+                        vals[0] += b0.x; vals[1] += b0.y; vals[2] += b0.z; vals[3] += b0.w;
+                        vals[4] += b1.x; vals[5] += b1.y; vals[6] += b1.z; vals[7] += b1.w;
+                    }
+                    if (prm.act == MF_ACT_GELU) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) vals[i] = gelu_erf(vals[i]);
+                    }
+                    if (prm.residual) {
+                        const uint32_t rr[4] = {myres[j].x, myres[j].y, myres[j].z, myres[j].w};
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            vals[2 * i] += __uint_as_float(rr[i] << 16);
+                            vals[2 * i + 1] += __uint_as_float(rr[i] & 0xffff0000u);
+                        }
+                    }
+                    uint4 o;
+                    o.x = ptx::pack_bf16(vals[0], vals[1]);
+                    o.y = ptx::pack_bf16(vals[2], vals[3]);
+                    o.z = ptx::pack_bf16(vals[4], vals[5]);
+                    o.w = ptx::pack_bf16(vals[6], vals[7]);
+                    stage[lane * 8 + (j ^ (lane & 7))] = o;
+                }
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int r = 4 * i + crow;
+                    if (row0 + r < prm.M)
+                        *reinterpret_cast<uint4*>(dst + static_cast<size_t>(row0 + r) * prm.n_split + 64 * g + 8 * cchunk) =
+                            stage[r * 8 + (cchunk ^ (r & 7))];
+                }
+                __syncwarp();
             }
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&sm.acc_empty[buf]);
         }
     }
     ptx::tc_fence_before();
