@@ -47,3 +47,31 @@ def split_heads(y, heads, head_dim):
     m = y.shape[0]
     hd = heads * head_dim
     return tuple(y[:, i * hd:(i + 1) * hd].reshape(m, heads, head_dim) for i in range(3))
+
+
+def round_bf16(a):
+    """E5: every tensor stored between two layers is bf16, rounded to nearest even (BJ: "bf16 tokens").
+    fp64 -> fp32 (nearest even) -> keep the top 16 bits with round-to-nearest-even on the dropped 16."""
+    f = np.asarray(a, dtype=np.float64).astype(np.float32)
+    bits = f.view(np.uint32).astype(np.uint64)
+    rounded = ((bits + 0x7FFF + ((bits >> 16) & 1)) >> 16) << 16
+    out = rounded.astype(np.uint32).view(np.float32).astype(np.float64)
+    return np.where(np.isfinite(f), out, f.astype(np.float64))
+
+
+def block_forward(x, wts, frames_per_window, tokens_per_frame, heads, mode, attention_fn, store=round_bf16):
+    """E1 + E2 for one window: x [S, d] -> y [S, d], S = W*P.  `wts` maps ln1_g, ln1_b, w_qkv, b_qkv, w_o, b_o, ln2_g,
+    ln2_b, w_1, b_1, w_2, b_2 to arrays.  `attention_fn(q, k, v, W, P, mode)` is oracle.attention.window_attention
+    (passed in so that this module stays a leaf).  `store` is applied to every tensor the method keeps between two
+    layers (E5); pass `lambda a: a` for the unrounded mathematical block."""
+    x = np.asarray(x, dtype=np.float64)
+    s_len, d = x.shape
+    hd = d // heads
+    a = store(layernorm(x, wts["ln1_g"], wts["ln1_b"]))
+    q, k, v = (store(t) for t in split_heads(linear(a, wts["w_qkv"], wts["b_qkv"]), heads, hd))
+    o, _ = attention_fn(q[None], k[None], v[None], frames_per_window, tokens_per_frame, mode)
+    o = store(o[0].reshape(s_len, d))
+    h = store(linear(o, wts["w_o"], wts["b_o"]) + x)
+    m = store(layernorm(h, wts["ln2_g"], wts["ln2_b"]))
+    u = store(gelu(linear(m, wts["w_1"], wts["b_1"])))
+    return store(linear(u, wts["w_2"], wts["b_2"]) + h)

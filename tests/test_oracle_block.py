@@ -62,3 +62,42 @@ def test_split_heads_layout():
     q, k, v = ob.split_heads(y, heads, hd)
     assert q.shape == (2, heads, hd)
     assert q[1, 2, 3] == y[1, 2 * hd + 3] and k[0, 1, 0] == y[0, heads * hd + hd] and v[1, 0, 1] == y[1, 2 * heads * hd + 1]
+
+
+def test_round_bf16_matches_torch_and_ties_to_even():
+    rng = np.random.default_rng(5)
+    a = np.concatenate([rng.standard_normal(4096) * 10.0 ** rng.integers(-6, 6, 4096), [0.0, -0.0, 1.0, 65504.0]])
+    ref = torch.from_numpy(a).to(torch.float32).to(torch.bfloat16).to(torch.float64).numpy()
+    assert np.array_equal(ob.round_bf16(a), ref)
+    # 1 + 2^-8 is exactly half way between 1 and 1 + 2^-7: ties go to the even mantissa
+    assert ob.round_bf16(1.0 + 2.0 ** -8) == 1.0 and ob.round_bf16(1.0 + 3 * 2.0 ** -8) == 1.0 + 2.0 ** -6
+
+
+def test_block_forward_identity_cases():
+    from oracle import attention as oa
+    rng = np.random.default_rng(6)
+    s_len, d, heads = 12, 8, 2
+    x = rng.standard_normal((s_len, d))
+    z = lambda *shape: np.zeros(shape)
+    wts = dict(ln1_g=np.ones(d), ln1_b=z(d), w_qkv=rng.standard_normal((3 * d, d)), b_qkv=z(3 * d), w_o=z(d, d), b_o=z(d),
+               ln2_g=np.ones(d), ln2_b=z(d), w_1=rng.standard_normal((4 * d, d)), b_1=z(4 * d), w_2=z(d, 4 * d), b_2=z(d))
+    ident = lambda a: a
+    # zero output projections: both residual branches vanish, the block is the identity
+    assert np.array_equal(ob.block_forward(x, wts, 3, 4, heads, oa.GLOBAL, oa.window_attention, store=ident), x)
+    # only biases on the two branches: y = x + b_o + b_2
+    wts["b_o"], wts["b_2"] = rng.standard_normal(d), rng.standard_normal(d)
+    y = ob.block_forward(x, wts, 3, 4, heads, oa.GLOBAL, oa.window_attention, store=ident)
+    assert np.abs(y - (x + wts["b_o"] + wts["b_2"])).max() < 1e-14
+    # w_v = I-selecting, w_o = I, uniform attention (w_q = w_k = 0): branch 1 adds the mean over tokens of LN1(x)
+    wq = z(3 * d, d); wq[2 * d:] = np.eye(d)
+    wts.update(w_qkv=wq, w_o=np.eye(d), b_o=z(d), b_2=z(d))
+    y = ob.block_forward(x, wts, 3, 4, heads, oa.GLOBAL, oa.window_attention, store=ident)
+    ln = ob.layernorm(x, np.ones(d), z(d))
+    assert np.abs(y - (x + ln.mean(axis=0, keepdims=True))).max() < 1e-13
+    # frame mode: the mean is taken per frame of 4 tokens
+    y = ob.block_forward(x, wts, 3, 4, heads, oa.FRAME, oa.window_attention, store=ident)
+    per_frame = np.repeat(ln.reshape(3, 4, d).mean(axis=1), 4, axis=0)
+    assert np.abs(y - (x + per_frame)).max() < 1e-13
+    # bf16 storage only perturbs the result at the 2^-8 level
+    yb = ob.block_forward(x, wts, 3, 4, heads, oa.FRAME, oa.window_attention)
+    assert 0 < np.abs(yb - y).max() < 0.05
