@@ -186,6 +186,30 @@ mf_status mf_linear(const void* x, const void* w, const float* bias, const void*
 mf_status mf_layernorm(const void* x, const float* gamma, const float* beta, float eps, void* out, int M,
                        int d, void* stream);
 
+/* One pre-norm transformer block around the window attention (reading E1, E2, E5 in DESIGN.md):
+ *   h = x + W_o Attn(split_heads(W_qkv LN1(x) + b_qkv)) + b_o ;  y = h + W_2 GELU(W_1 LN2(h) + b_1) + b_2
+ * x, y: bf16 [windows * W * P, heads * head_dim] (token order as in mf_window_attention); y may equal x (in place).
+ * Weights are nn.Linear-layout bf16 matrices and fp32 vectors (all device memory, 16-byte aligned):
+ *   w_qkv [3 d, d] (rows: q | k | v, each head-major), w_o [d, d], w_1 [d_hidden, d], w_2 [d, d_hidden].
+ * Every tensor kept between two kernels is bf16 (E5).  Seven launches: layernorm, linear (q|k|v), window attention,
+ * linear (+residual), layernorm, linear (+GELU), linear (+residual).  d = heads * head_dim must be 256, 512, 768 or
+ * 1024 with head_dim 64, d_hidden % 256 == 0.  workspace: mf_block_workspace_size() bytes of device memory.
+ */
+typedef struct {
+    const float* ln1_gamma; const float* ln1_beta;
+    const void* w_qkv;      const float* b_qkv;
+    const void* w_o;        const float* b_o;
+    const float* ln2_gamma; const float* ln2_beta;
+    const void* w_1;        const float* b_1;
+    const void* w_2;        const float* b_2;
+} mf_block_weights;
+
+size_t mf_block_workspace_size(int windows, int frames_per_window, int tokens_per_frame, int d_model, int d_hidden);
+
+mf_status mf_block_forward(const void* x, const mf_block_weights* weights, void* y, int windows,
+                           int frames_per_window, int tokens_per_frame, int heads, int head_dim, int d_hidden,
+                           mf_attn_mode mode, float ln_eps, void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,8 @@ ACT_NONE, ACT_GELU = 0, 1
 
 EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
-           "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm"]
+           "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
+           "mf_block_workspace_size", "mf_block_forward"]
 
 
 class MfError(RuntimeError):
@@ -28,6 +29,11 @@ class MfError(RuntimeError):
 
 class Intrinsics(ctypes.Structure):
     _fields_ = [("fx", ctypes.c_double), ("fy", ctypes.c_double), ("cx", ctypes.c_double), ("cy", ctypes.c_double)]
+
+
+class BlockWeights(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in ("ln1_gamma", "ln1_beta", "w_qkv", "b_qkv", "w_o", "b_o", "ln2_gamma", "ln2_beta",
+                                               "w_1", "b_1", "w_2", "b_2")]
 
 
 class FocusParams(ctypes.Structure):
@@ -64,6 +70,9 @@ def lib():
                                               ctypes.POINTER(FocusParams), vp, vp, vp, vp, vp, vp]
         L.mf_linear.argtypes = [vp, vp, vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp]
         L.mf_layernorm.argtypes = [vp, vp, vp, cf, vp, ci, ci, vp]
+        L.mf_block_workspace_size.restype = ctypes.c_size_t
+        L.mf_block_workspace_size.argtypes = [ci, ci, ci, ci, ci]
+        L.mf_block_forward.argtypes = [vp, ctypes.POINTER(BlockWeights), vp, ci, ci, ci, ci, ci, ci, ci, cf, vp, ctypes.c_size_t, vp]
         _lib = L
     return _lib
 
@@ -246,4 +255,25 @@ def layernorm(x, gamma, beta, eps=1e-6, out=None):
         out = torch.empty_like(x)
     _dev(out, torch.bfloat16, "out")
     _check(lib().mf_layernorm(_ptr(x), _ptr(gamma), _ptr(beta), float(eps), _ptr(out), x.shape[0], x.shape[1], _stream()))
+    return out
+
+
+_BLOCK_KEYS = ("ln1_g", "ln1_b", "w_qkv", "b_qkv", "w_o", "b_o", "ln2_g", "ln2_b", "w_1", "b_1", "w_2", "b_2")
+
+
+def block_forward(x, wts, windows, frames_per_window, tokens_per_frame, heads, mode=ATTN_GLOBAL, ln_eps=1e-6,
+                  out=None, workspace=None):
+    """One pre-norm transformer block (mf_block_forward).  x bf16 [windows*W*P, d]; wts: dict with the keys of
+    _BLOCK_KEYS (bf16 matrices, fp32 vectors, biases may be None)."""
+    _dev(x, torch.bfloat16, "x")
+    d = x.shape[1]
+    d_hidden = wts["w_1"].shape[0]
+    need = lib().mf_block_workspace_size(windows, frames_per_window, tokens_per_frame, d, d_hidden)
+    if workspace is None:
+        workspace = torch.empty((need,), device=x.device, dtype=torch.uint8)
+    if out is None:
+        out = torch.empty_like(x)
+    bw = BlockWeights(*[0 if wts.get(k) is None else wts[k].data_ptr() for k in _BLOCK_KEYS])
+    _check(lib().mf_block_forward(_ptr(x), ctypes.byref(bw), _ptr(out), windows, frames_per_window, tokens_per_frame, heads,
+                                  d // heads, d_hidden, mode, float(ln_eps), _ptr(workspace), workspace.numel(), _stream()))
     return out

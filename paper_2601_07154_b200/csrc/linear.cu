@@ -377,3 +377,45 @@ extern "C" mf_status mf_layernorm(const void* x, const float* gamma, const float
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// One transformer block (reading E1, E2, E5): host-side sequencing of the seven launches
+// ------------------------------------------------------------------------------------------------
+static size_t block_tokens_bytes(long long tokens, int width) { return (static_cast<size_t>(tokens) * width * 2 + 255) / 256 * 256; }
+
+extern "C" size_t mf_block_workspace_size(int windows, int frames_per_window, int tokens_per_frame, int d_model, int d_hidden) {
+    if (windows < 1 || frames_per_window < 1 || tokens_per_frame < 1 || d_model < 1 || d_hidden < 1) return 0;
+    const long long tokens = static_cast<long long>(windows) * frames_per_window * tokens_per_frame;
+    return 6 * block_tokens_bytes(tokens, d_model) + block_tokens_bytes(tokens, d_hidden);     // a, q, k, v, o, h | u
+}
+
+extern "C" mf_status mf_block_forward(const void* x, const mf_block_weights* wt, void* y, int windows, int frames_per_window,
+                                      int tokens_per_frame, int heads, int head_dim, int d_hidden, mf_attn_mode mode,
+                                      float ln_eps, void* workspace, size_t workspace_bytes, void* stream) {
+    using namespace mf;
+    if (!x || !wt || !y) return fail(MF_ERR_INVALID_ARG, "mf_block_forward: NULL tensor");
+    if (windows < 1 || frames_per_window < 1 || tokens_per_frame < 1 || heads < 1 || head_dim < 1 || d_hidden < 1)
+        return fail(MF_ERR_INVALID_ARG, "mf_block_forward: non-positive dimension");
+    if (!wt->ln1_gamma || !wt->ln1_beta || !wt->w_qkv || !wt->w_o || !wt->ln2_gamma || !wt->ln2_beta || !wt->w_1 || !wt->w_2)
+        return fail(MF_ERR_INVALID_ARG, "mf_block_forward: NULL weight");
+    const int d = heads * head_dim;
+    const long long tokens_ll = static_cast<long long>(windows) * frames_per_window * tokens_per_frame;
+    if (tokens_ll > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_block_forward: too many tokens");
+    const int tokens = static_cast<int>(tokens_ll);
+    const size_t need = mf_block_workspace_size(windows, frames_per_window, tokens_per_frame, d, d_hidden);
+    if (!workspace || workspace_bytes < need || !aligned16(workspace))
+        return fail(MF_ERR_WORKSPACE, "mf_block_forward: workspace needs %zu bytes (got %zu)", need, workspace_bytes);
+    char* base = static_cast<char*>(workspace);
+    const size_t td = block_tokens_bytes(tokens, d);
+    void *a = base, *q = base + td, *k = base + 2 * td, *v = base + 3 * td, *o = base + 4 * td, *h = base + 5 * td, *u = base + 6 * td;
+    mf_status st;
+    if ((st = mf_layernorm(x, wt->ln1_gamma, wt->ln1_beta, ln_eps, a, tokens, d, stream)) != MF_OK) return st;
+    if ((st = mf_linear(a, wt->w_qkv, wt->b_qkv, nullptr, q, k, v, tokens, 3 * d, d, d, MF_ACT_NONE, stream)) != MF_OK) return st;
+    if ((st = mf_window_attention(q, k, v, o, nullptr, windows, frames_per_window, tokens_per_frame, heads, head_dim, mode, 0.f,
+                                  stream)) != MF_OK) return st;
+    if ((st = mf_linear(o, wt->w_o, wt->b_o, x, h, nullptr, nullptr, tokens, d, d, d, MF_ACT_NONE, stream)) != MF_OK) return st;
+    if ((st = mf_layernorm(h, wt->ln2_gamma, wt->ln2_beta, ln_eps, a, tokens, d, stream)) != MF_OK) return st;
+    if ((st = mf_linear(a, wt->w_1, wt->b_1, nullptr, u, nullptr, nullptr, tokens, d_hidden, d, d_hidden, MF_ACT_GELU, stream)) != MF_OK)
+        return st;
+    return mf_linear(u, wt->w_2, wt->b_2, h, y, nullptr, nullptr, tokens, d, d_hidden, d, MF_ACT_NONE, stream);
+}

@@ -148,3 +148,15 @@ def linear_inputs(m, n, k, seed, device="cpu"):
     w = (torch.randn((n, k), generator=g, device=device, dtype=torch.float32) / (k ** 0.5)).to(torch.bfloat16)
     b = 0.1 * torch.randn((n,), generator=g, device=device, dtype=torch.float32)
     return x, w, b
+
+
+def block_weights(d, d_hidden, seed, device="cpu"):
+    """Seeded synthetic weights of one pre-norm block (stand-in for trained weights): matrices ~ N(0, 1/fan_in) bf16,
+    biases ~ N(0, 0.1) fp32, LayerNorm gamma ~ 1 + N(0, 0.1), beta ~ N(0, 0.1) fp32."""
+    import torch
+    g = torch.Generator(device=device).manual_seed(int(seed))
+    rn = lambda *shape: torch.randn(shape, generator=g, device=device, dtype=torch.float32)
+    mat = lambda n, k: (rn(n, k) / (k ** 0.5)).to(torch.bfloat16)
+    return dict(ln1_g=1 + 0.1 * rn(d), ln1_b=0.1 * rn(d), w_qkv=mat(3 * d, d), b_qkv=0.1 * rn(3 * d), w_o=mat(d, d),
+                b_o=0.1 * rn(d), ln2_g=1 + 0.1 * rn(d), ln2_b=0.1 * rn(d), w_1=mat(d_hidden, d), b_1=0.1 * rn(d_hidden),
+                w_2=mat(d, d_hidden), b_2=0.1 * rn(d))

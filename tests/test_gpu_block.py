@@ -95,3 +95,32 @@ def test_linear_errors(api):
     x3, w3, _ = synth.linear_inputs(64, 256, 48, seed=1, device="cuda")
     with pytest.raises(api.MfError):
         api.linear(x3, w3)                                          # K % 64 != 0
+
+
+@pytest.mark.parametrize("mode_name", ["global", "frame"])
+@pytest.mark.parametrize("windows,w,p,heads,d_hidden", [(2, 2, 100, 4, 1024), (1, 3, 77, 8, 768)])
+def test_block_forward_vs_oracle(api, windows, w, p, heads, d_hidden, mode_name):
+    # whole pre-norm block (E1, E2) with bf16 storage between kernels (E5): 7 launches vs oracle.block.block_forward.
+    # Intermediate bf16 tensors may differ from the oracle's by rare 1-ulp rounding flips (fp32 vs fp64 sums landing on
+    # either side of a rounding boundary); a flipped h plus y's own rounding is 2 bf16 ulps = 2^-6 |ref| on a few elements.
+    from oracle import attention as oa
+    mode = oa.GLOBAL if mode_name == "global" else oa.FRAME
+    d = heads * 64
+    s_len = w * p
+    x = synth.tokens(windows * s_len, d, seed=7 + windows + heads, device="cuda")
+    wts = synth.block_weights(d, d_hidden, seed=11 + heads, device="cuda")
+    y = api.block_forward(x, wts, windows, w, p, heads, mode)
+    torch.cuda.synchronize()
+    w64 = {k: _to64(v) for k, v in wts.items()}
+    for n in range(windows):
+        ref = ob.block_forward(_to64(x[n * s_len:(n + 1) * s_len]), w64, w, p, heads, mode, oa.window_attention)
+        got = _to64(y[n * s_len:(n + 1) * s_len])
+        dlt = got - ref
+        assert np.isfinite(got).all()
+        # (a flip of h is one ulp of |h|, which can exceed |y| where the MLP branch cancels h: hence the max|ref| term)
+        assert (np.abs(dlt) <= 2.0 ** -6 * np.abs(ref) + 2.0 ** -7 * np.abs(ref).max()).all(), float(np.abs(dlt).max())
+        assert np.linalg.norm(dlt) / np.linalg.norm(ref) <= 4e-3
+    # in place (y == x) gives the same bits
+    x2 = x.clone()
+    api.block_forward(x2, wts, windows, w, p, heads, mode, out=x2)
+    assert torch.equal(x2, y)
