@@ -33,6 +33,7 @@ def parse_args():
     ap.add_argument("--max-windows", type=int, default=0, help="debug: truncate the clip to this many windows")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-block", action="store_true", help="skip the whole-transformer-block measurement (SURVEY 8(f) NEXT-1)")
     return ap.parse_args()
 
 
@@ -215,6 +216,38 @@ class Workload:
                                           "global_w2c": self.hout["global_w2c"]})
 
 
+def measure_block(wl, torch, api):
+    """SURVEY 8(f) NEXT-1 (not part of the headline step): one FRAME + one GLOBAL pre-norm transformer block
+    (mf_block_forward: LN, QKV GEMM, window attention, out-proj GEMM + residual, LN, fc1 GEMM + GELU, fc2 GEMM + residual)
+    on one launch batch of windows, d = H*D, hidden = 4d, seeded synthetic weights."""
+    from paper_2601_07154_b200 import synth
+    d, dh = wl.H * wl.D, 4 * wl.H * wl.D
+    tokens = wl.B * wl.S
+    x = synth.tokens(tokens, d, synth.seed_for(wl.cfg_idx, 6), device=wl.device)
+    wts = synth.block_weights(d, dh, synth.seed_for(wl.cfg_idx, 7), device=wl.device)
+    need = api.lib().mf_block_workspace_size(wl.B, wl.W, wl.P, d, dh)
+    ws = torch.empty((need,), device=wl.device, dtype=torch.uint8)
+    y = torch.empty_like(x)
+    gemm_flops = 2.0 * tokens * (3 * d * d + d * d + 2 * d * dh)
+    out = {"what": "mf_block_forward on one launch batch (SURVEY 8(f) NEXT-1; not in the headline step)",
+           "tokens": tokens, "d_model": d, "d_hidden": dh, "gemm_flops_per_block": gemm_flops}
+    for name, mode, aflops in (("frame", api.ATTN_FRAME, wl.flops_frame), ("global", api.ATTN_GLOBAL, wl.flops_global)):
+        for _ in range(2):
+            api.block_forward(x, wts, wl.B, wl.W, wl.P, wl.H, mode, out=y, workspace=ws)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            api.block_forward(x, wts, wl.B, wl.W, wl.P, wl.H, mode, out=y, workspace=ws)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 3
+        out[name + "_block_ms"] = ms
+        out[name + "_block_tflops"] = (gemm_flops + aflops * wl.B) / (ms * 1e-3) / 1e12
+    pair_ms = out["frame_block_ms"] + out["global_block_ms"]
+    out["frames_per_s_full_blocks"] = wl.N / (pair_ms * 1e-3 * (wl.layers // 2) * ((wl.Nw + wl.B - 1) // wl.B))
+    return out
+
+
 def oracle_sample(cfg_idx, wl_dims, rows=1024):
     """Times the oracle, as it stands, on a bounded sample of the same workload (host cores) and
     extrapolates to the whole clip.  Returns (frames_per_s, seconds_of_sample, description, cores)."""
@@ -385,6 +418,10 @@ def main():
         fps, secs, desc, cores = oracle_sample(args.config, dims)
         cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc, "sample_seconds": secs}
 
+    block = None
+    if rank == 0 and not args.no_block and wl.layers > 1:
+        block = measure_block(wl, torch, api)
+
     if rank == 0:
         dims = dims_of(args.config, args)
         line = {"metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)", "value": value,
@@ -392,7 +429,7 @@ def main():
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
                 "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
-                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+                "cpu_baseline": cpu, "e2e": e2e, "block": block, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
         print(json.dumps(line))
     replicas.finish()
 
