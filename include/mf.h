@@ -87,6 +87,19 @@ typedef enum { MF_ALIGN_YAW_TRANSLATION = 0, MF_ALIGN_RIGID = 1 } mf_align_mode;
 mf_status mf_chain_poses(const float* local_w2c, int sequences, int num_windows, int W, int stride,
                          int num_frames, mf_align_mode mode, double* global_w2c, void* stream);
 
+/* Streaming form of the pose chain (each batch is aligned "incrementally" to the terminal pose of the trajectory
+ * so far).  One window per call; the state (A_{n-1} and the previous window's last local pose,
+ * mf_chain_state_size() bytes of device memory, 8-byte aligned, contents irrelevant before the first window) is
+ * updated in place.  first_window != 0: A_0 = I, all W frames are emitted.  Otherwise the window shares its first
+ * W - new_frames frames with the previous window (new_frames = start_n - start_{n-1}, so 1 <= new_frames < W), it is
+ * anchored at its local frame W - new_frames - 1 (= the previous window's last frame) and its last new_frames frames
+ * are emitted.  out_w2c: fp64 [emitted, 4, 4].  Same operations in the same order as mf_chain_poses: feeding the
+ * windows of a clip one by one reproduces its output bit for bit.
+ */
+size_t mf_chain_state_size(void);
+mf_status mf_chain_poses_step(const float* window_local_w2c, void* state, int W, int new_frames, int first_window,
+                              mf_align_mode mode, double* out_w2c, void* stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Motion focus (Eq. 1-7) and motion-guided depth (Fig. 1(iii), Fig. 5).
  *

@@ -20,7 +20,7 @@ ACT_NONE, ACT_GELU = 0, 1
 EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
            "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
-           "mf_block_workspace_size", "mf_block_forward"]
+           "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step"]
 
 
 class MfError(RuntimeError):
@@ -73,6 +73,8 @@ def lib():
         L.mf_block_workspace_size.restype = ctypes.c_size_t
         L.mf_block_workspace_size.argtypes = [ci, ci, ci, ci, ci]
         L.mf_block_forward.argtypes = [vp, ctypes.POINTER(BlockWeights), vp, ci, ci, ci, ci, ci, ci, ci, cf, vp, ctypes.c_size_t, vp]
+        L.mf_chain_state_size.restype = ctypes.c_size_t
+        L.mf_chain_poses_step.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
         _lib = L
     return _lib
 
@@ -276,4 +278,21 @@ def block_forward(x, wts, windows, frames_per_window, tokens_per_frame, heads, m
     bw = BlockWeights(*[0 if wts.get(k) is None else wts[k].data_ptr() for k in _BLOCK_KEYS])
     _check(lib().mf_block_forward(_ptr(x), ctypes.byref(bw), _ptr(out), windows, frames_per_window, tokens_per_frame, heads,
                                   d // heads, d_hidden, mode, float(ln_eps), _ptr(workspace), workspace.numel(), _stream()))
+    return out
+
+
+def chain_state(device="cuda"):
+    """Device-resident state of the streaming pose chain (mf_chain_poses_step)."""
+    return torch.zeros((lib().mf_chain_state_size(),), device=device, dtype=torch.uint8)
+
+
+def chain_poses_step(window_local_w2c, state, new_frames=0, first=False, mode=ALIGN_YAW_TRANSLATION, out=None):
+    """One window [W,4,4] fp32 through the incremental anchoring; returns the emitted global poses fp64 [n,4,4]."""
+    _dev(window_local_w2c, torch.float32, "window_local_w2c")
+    w = window_local_w2c.shape[0]
+    n = w if first else new_frames
+    if out is None:
+        out = torch.empty((max(n, 0), 4, 4), device=window_local_w2c.device, dtype=torch.float64)
+    _check(lib().mf_chain_poses_step(_ptr(window_local_w2c), _ptr(state), w, int(new_frames), 1 if first else 0, mode, _ptr(out),
+                                     _stream()))
     return out

@@ -113,6 +113,64 @@ chain_poses_kernel(const float* __restrict__ local_w2c, int num_windows, int W, 
     }
 }
 
+// Streaming form ("incremental"): one window per call, A_{n-1} and the previous window's terminal local pose
+// carried in a small device-resident state.  Same operations in the same order as chain_poses_kernel: bit-identical.
+struct ChainState {
+    double a[12];           // A_{n-1}: rotation rows then translation
+    float prev_last[16];    // T^{L_{n-1} -> c}_{W-1}
+    int windows_seen;
+    int pad[3];
+};
+
+__global__ void __launch_bounds__(128)
+chain_step_kernel(const float* __restrict__ win, ChainState* __restrict__ state, int W, int new_frames, int first, int mode,
+                  double* __restrict__ out) {
+    __shared__ double s_ai[12];
+    const int emit_from = first ? 0 : W - new_frames;
+    if (threadIdx.x == 0) {
+        Rigid a = rigid_identity();
+        if (!first) {
+#pragma unroll
+            for (int i = 0; i < 9; ++i) a.r[i] = state->a[i];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) a.t[i] = state->a[9 + i];
+            const Rigid b = boundary(load_local(state->prev_last), load_local(win + static_cast<size_t>(emit_from - 1) * 16), mode);
+            a = rigid_compose(a, b);
+        }
+        const Rigid ai = rigid_inverse(a);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) {
+            s_ai[i] = ai.r[i];
+            state->a[i] = a.r[i];
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            s_ai[9 + i] = ai.t[i];
+            state->a[9 + i] = a.t[i];
+        }
+        state->windows_seen = first ? 1 : state->windows_seen + 1;
+    }
+    __syncthreads();
+    if (threadIdx.x < 16) state->prev_last[threadIdx.x] = win[static_cast<size_t>(W - 1) * 16 + threadIdx.x];
+    Rigid ai;
+#pragma unroll
+    for (int i = 0; i < 9; ++i) ai.r[i] = s_ai[i];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) ai.t[i] = s_ai[9 + i];
+    for (int k = emit_from + threadIdx.x; k < W; k += blockDim.x) {
+        const Rigid g = rigid_compose(load_local(win + static_cast<size_t>(k) * 16), ai);
+        double* o = out + static_cast<size_t>(k - emit_from) * 16;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            o[4 * i + 0] = g.r[3 * i + 0];
+            o[4 * i + 1] = g.r[3 * i + 1];
+            o[4 * i + 2] = g.r[3 * i + 2];
+            o[4 * i + 3] = g.t[i];
+        }
+        o[12] = 0.0; o[13] = 0.0; o[14] = 0.0; o[15] = 1.0;
+    }
+}
+
 }  // namespace mf
 
 extern "C" mf_status mf_chain_poses(const float* local_w2c, int sequences, int num_windows, int W, int stride,
@@ -138,6 +196,26 @@ extern "C" mf_status mf_chain_poses(const float* local_w2c, int sequences, int n
                                         static_cast<int>(smem)));
     mf::chain_poses_kernel<<<sequences, 256, smem, static_cast<cudaStream_t>(stream)>>>(
         local_w2c, num_windows, W, stride, num_frames, static_cast<int>(mode), global_w2c);
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}
+
+extern "C" size_t mf_chain_state_size(void) { return sizeof(mf::ChainState); }
+
+extern "C" mf_status mf_chain_poses_step(const float* window_local_w2c, void* state, int W, int new_frames, int first_window,
+                                         mf_align_mode mode, double* out_w2c, void* stream) {
+    if (!window_local_w2c || !state || !out_w2c) return mf::fail(MF_ERR_INVALID_ARG, "mf_chain_poses_step: NULL pointer");
+    if (W < 1) return mf::fail(MF_ERR_INVALID_ARG, "mf_chain_poses_step: W=%d", W);
+    if (!first_window && (new_frames < 1 || new_frames >= W))
+        return mf::fail(MF_ERR_INVALID_ARG, "mf_chain_poses_step: need 1 <= new_frames < W (overlap >= 1), got %d", new_frames);
+    if (mode != MF_ALIGN_YAW_TRANSLATION && mode != MF_ALIGN_RIGID)
+        return mf::fail(MF_ERR_INVALID_ARG, "mf_chain_poses_step: bad mode %d", static_cast<int>(mode));
+    if ((reinterpret_cast<uintptr_t>(state) & 7u) != 0) return mf::fail(MF_ERR_ALIGNMENT, "mf_chain_poses_step: state must be 8-byte aligned");
+    mf_status st = mf::require_sm100();
+    if (st != MF_OK) return st;
+    mf::chain_step_kernel<<<1, 128, 0, static_cast<cudaStream_t>(stream)>>>(window_local_w2c, static_cast<mf::ChainState*>(state), W,
+                                                                           new_frames, first_window ? 1 : 0, static_cast<int>(mode),
+                                                                           out_w2c);
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
 }

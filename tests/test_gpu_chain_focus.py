@@ -42,6 +42,28 @@ def test_chain_bit_exact(api, cfg_idx, n_frames, w, stride, mode):
     assert np.array_equal(got, ref), f"max diff {np.abs(got - ref).max()}"
 
 
+@pytest.mark.parametrize("mode", [oc.YAW_TRANSLATION, oc.RIGID])
+@pytest.mark.parametrize("cfg_idx,n_frames,w,stride", [(3, 200, 32, 16), (1, 23, 8, 7), (1, 9, 4, 1), (4, 720, 64, 32)])
+def test_chain_streaming_matches_batch_bit_for_bit(api, cfg_idx, n_frames, w, stride, mode):
+    # mf_chain_poses_step ("incremental"): one window per call, state carried on the device
+    from oracle import windows as ow
+    cfg = synth.CONFIGS[cfg_idx]
+    traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
+    loc = synth.local_windows(traj, w, stride, seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    ref = np.array(oc.chain_poses(loc.tolist(), w, stride, n_frames, mode))
+    dloc = torch.from_numpy(loc).cuda()
+    state = api.chain_state()
+    state.fill_(0xAB)                                        # contents before the first window are irrelevant
+    starts = ow.window_starts(n_frames, w, stride)
+    outs = []
+    for n, st in enumerate(starts):
+        outs.append(api.chain_poses_step(dloc[n], state, new_frames=0 if n == 0 else st - starts[n - 1], first=n == 0, mode=mode))
+    got = torch.cat(outs).cpu().numpy()
+    assert got.shape == ref.shape and np.array_equal(got, ref)
+    with pytest.raises(api.MfError):
+        api.chain_poses_step(dloc[0], state, new_frames=w)  # no overlap
+
+
 def test_chain_multi_sequence_and_errors(api):
     cfg = synth.CONFIGS[1]
     traj = [synth.trajectory(cfg, synth.seed_for(1, 10 + i), 40) for i in range(3)]
