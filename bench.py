@@ -33,6 +33,7 @@ def parse_args():
     ap.add_argument("--max-windows", type=int, default=0, help="debug: truncate the clip to this many windows")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stream", action="store_true", help="skip the per-window streaming latency measurement (SURVEY 8(f) NEXT-2)")
     ap.add_argument("--no-block", action="store_true", help="skip the whole-transformer-block measurement (SURVEY 8(f) NEXT-1)")
     return ap.parse_args()
 
@@ -271,6 +272,71 @@ def measure_block(wl, torch, api):
     return out
 
 
+def measure_streaming(wl, torch, api):
+    """SURVEY 8(f) NEXT-2 (not part of the headline step): the path one window at a time, as a stream would see it.
+    Per window: its q,k,v into static buffers, 24 attention launches, mf_chain_poses_step, the new poses appended to a
+    rolling pose buffer, mf_motion_focus for the `stride` new frames.  Timed eagerly and as one replayed CUDA graph."""
+    c, dev = wl.cfg, wl.device
+    m = wl.stride
+    ring_len = wl.W + 32
+    q, k, v = (torch.empty_like(t[:1]) for t in (wl.q, wl.k, wl.v))
+    o = [torch.empty_like(q) for _ in range(2)]
+    win = torch.empty((wl.W, 4, 4), device=dev, dtype=torch.float32)
+    state = api.chain_state(dev)
+    ring = torch.zeros((ring_len, 4, 4), device=dev, dtype=torch.float64)
+    new = torch.empty((m, 4, 4), device=dev, dtype=torch.float64)
+    depth = wl.depth[:m]
+    fmap, guided = torch.empty_like(depth), torch.empty_like(depth)
+    ws = torch.empty((api.lib().mf_motion_focus_workspace_size(m, wl.width, wl.height, wl.n_points),), device=dev, dtype=torch.uint8)
+
+    def load(n):
+        q.copy_(wl.q[n:n + 1]); k.copy_(wl.k[n:n + 1]); v.copy_(wl.v[n:n + 1]); win.copy_(wl.local[n])
+
+    def step(first=False):
+        for layer in range(wl.layers):
+            api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_FRAME if layer % 2 == 0 else api.ATTN_GLOBAL, out=o[layer % 2])
+        if first:
+            full = api.chain_poses_step(win, state, first=True)
+            ring[-wl.W:].copy_(full)
+            return
+        api.chain_poses_step(win, state, new_frames=m, out=new)
+        ring.copy_(torch.cat([ring[m:], new]))
+        api.motion_focus(ring, c["fx"], c["fy"], c["cx"], c["cy"], wl.width, wl.height, wl.params, depth=depth,
+                         render_begin=ring_len - m, render_end=ring_len, workspace=ws,
+                         out={"focus_map": fmap, "guided_depth": guided})
+
+    def timed(fn, windows):
+        ts = []
+        for n in windows:
+            load(n)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ts.sort()
+        return ts[len(ts) // 2]
+
+    load(0); step(first=True)
+    load(1); step()
+    torch.cuda.synchronize()
+    eager_ms = timed(step, range(2, 5))
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream(device=dev)
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()                                               # warm-up on the capture stream
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph_ms = timed(graph.replay, range(5, 8))
+    return {"what": "one window at a time (SURVEY 8(f) NEXT-2; not in the headline step): 24 attention launches + "
+                    "mf_chain_poses_step + rolling pose buffer + mf_motion_focus of the new frames",
+            "new_frames_per_window": m, "eager_ms_per_window": eager_ms, "graph_ms_per_window": graph_ms,
+            "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
+
+
 def oracle_sample(cfg_idx, wl_dims, rows=1024):
     """Times the oracle, as it stands, on a bounded sample of the same workload (host cores) and
     extrapolates to the whole clip.  Returns (frames_per_s, seconds_of_sample, description, cores)."""
@@ -445,6 +511,10 @@ def main():
     if rank == 0 and not args.no_block and wl.layers > 1:
         block = measure_block(wl, torch, api)
 
+    streaming = None
+    if rank == 0 and not args.no_stream and wl.Nw >= 8 and wl.layers > 1:
+        streaming = measure_streaming(wl, torch, api)
+
     if rank == 0:
         dims = dims_of(args.config, args)
         line = {"metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)", "value": value,
@@ -452,7 +522,7 @@ def main():
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
                 "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
-                "cpu_baseline": cpu, "e2e": e2e, "block": block, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+                "cpu_baseline": cpu, "e2e": e2e, "block": block, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
         print(json.dumps(line))
     replicas.finish()
 

@@ -64,6 +64,37 @@ def test_chain_streaming_matches_batch_bit_for_bit(api, cfg_idx, n_frames, w, st
         api.chain_poses_step(dloc[0], state, new_frames=w)  # no overlap
 
 
+def test_streaming_pipeline_matches_batch(api):
+    # chain step -> rolling pose buffer -> mf_motion_focus on the last `stride` frames == the batch pipeline, bit for bit
+    cfg = synth.CONFIGS[1]
+    n_frames, w, stride, n_points = 48, 8, 4, 15
+    width, height = 256, 128
+    k = (180.0, 180.0, 128.0, 64.0)
+    traj = synth.trajectory(cfg, synth.seed_for(1, 21), n_frames)
+    loc = torch.from_numpy(synth.local_windows(traj, w, stride, seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
+    depth = synth.depth(n_frames, height, width, 77, device="cuda")
+    prm = api.focus_params(n_points=n_points, sigma=12.0)
+    poses = api.chain_poses(loc, stride, n_frames)
+    batch = api.motion_focus(poses, *k, width, height, prm, depth=depth)
+    ring_len = w + 24                                        # >= n_points + 2 + stride frames of history
+    ring = torch.zeros((ring_len, 4, 4), device="cuda", dtype=torch.float64)
+    state = api.chain_state()
+    t_done = 0
+    for n in range(loc.shape[0]):
+        new = api.chain_poses_step(loc[n], state, new_frames=stride, first=n == 0)
+        m = new.shape[0]
+        ring = torch.cat([ring[m:], new])
+        t_done += m
+        if t_done < ring_len:                                # history not yet complete: the early frames are covered by the batch test
+            continue
+        out = api.motion_focus(ring, *k, width, height, prm, depth=depth[t_done - m:t_done], render_begin=ring_len - m,
+                               render_end=ring_len)
+        sl = slice(t_done - m, t_done)
+        assert torch.equal(out["focus_index"], batch["focus_index"][sl])
+        assert torch.equal(out["focus_map"], batch["focus_map"][sl]) and torch.equal(out["guided_depth"], batch["guided_depth"][sl])
+    assert t_done == n_frames
+
+
 def test_chain_multi_sequence_and_errors(api):
     cfg = synth.CONFIGS[1]
     traj = [synth.trajectory(cfg, synth.seed_for(1, 10 + i), 40) for i in range(3)]
