@@ -297,7 +297,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
                             ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
-                            if (((i >> 1) & 15) % 4 == 3 && ((i >> 1) & 15) / 4 < kPolyPairs) {
+                            if (((((i >> 1) & 15) * kPolyPairs) & 15) < kPolyPairs) {       // kPolyPairs of every 16 pairs, evenly spread
                                 exp2_poly2(s[c][i], s[c][i + 1]);
                             } else {
                                 s[c][i] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i])));
