@@ -331,7 +331,7 @@ def measure_streaming(wl, torch, api):
     torch.cuda.current_stream().wait_stream(side)
     torch.cuda.synchronize()
     graph_ms = timed(graph.replay, range(5, 8))
-    return {"what": "one window at a time (SURVEY 8(f) NEXT-2; not in the headline step): 24 attention launches + "
+    return {"what": f"one window at a time (SURVEY 8(f) NEXT-2; not in the headline step): {wl.layers} attention launches + "
                     "mf_chain_poses_step + rolling pose buffer + mf_motion_focus of the new frames",
             "new_frames_per_window": m, "eager_ms_per_window": eager_ms, "graph_ms_per_window": graph_ms,
             "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
@@ -394,7 +394,7 @@ def dims_of(cfg_idx, args):
 def config_block(cfg_idx, dims, args, extra=None):
     from paper_2601_07154_b200 import synth
     c = synth.CONFIGS[cfg_idx]
-    d = {"workload": f"BASELINE.json configs[{cfg_idx}] {c['name']}-shaped: W={dims['W']} stride={c['stride']} over "
+    d = {"workload": f"{'BASELINE.json configs[%d]' % cfg_idx if cfg_idx < 5 else 'extra workload (not in BASELINE.json)'} {c['name']}-shaped: W={dims['W']} stride={c['stride']} over "
                      f"{dims['N']} frames ({dims['Nw']} windows), P={dims['P']} tokens/frame, S={dims['S']}, "
                      f"{dims['layers']} alternating frame/global layers, H={dims['H']}, D={dims['D']}, bf16; "
                      f"focus map + guided depth at {c['width']}x{c['height']} fp32, N_points=15, sigma={c['sigma']}",

@@ -30,6 +30,12 @@ CONFIGS = [
     dict(name="town", W=64, stride=32, N=720, P=777, H=16, D=64, layers=24,
          width=3840, height=2160, fx=2800.0, fy=2800.0, cx=1920.0, cy=1080.0, fps=30,
          step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.05, sigma=20.0),
+    # Not a BASELINE.json config: the shape of the paper's own Table 2 row "DA3 Base, res 504, batch 60" as a second
+    # workload.  504 px at 16:9 with 14-px patches -> 36 x 20 = 720 tokens/frame; ViT-B widths
+    # (12 heads x 64, 12 blocks) are an ASSUMPTION about DA3 Base, not stated in PAPER.md; overlap W/2 as in BJ.
+    dict(name="table2-base-504-b60", W=60, stride=30, N=600, P=720, H=12, D=64, layers=12,
+         width=1920, height=1080, fx=1400.0, fy=1400.0, cx=960.0, cy=540.0, fps=30,
+         step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.15, sigma=20.0),
 ]
 
 
