@@ -150,6 +150,21 @@ def test_full_size_configs_sampled_rows(api, cfg_idx, windows, check):
             assert np.abs(g - lse_ref).max() <= 4e-3
 
 
+def _random_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    cases = []
+    for _ in range(n):
+        cases.append((int(rng.integers(1, 4)), int(rng.integers(1, 6)), int(rng.integers(1, 301)), int(rng.integers(1, 5)),
+                      int(rng.integers(0, 2)), float(rng.choice([1.0, 1.0, 2.0, 4.0])), int(rng.integers(0, 1 << 30))))
+    return cases
+
+
+@pytest.mark.parametrize("windows,w,p,heads,mode,qscale,seed", _random_cases(24, 20260107))
+def test_random_shapes(api, windows, w, p, heads, mode, qscale, seed):
+    # seeded random (windows, W, P, heads, mode, score scale): tiles, ragged tails and frame boundaries land anywhere
+    _check(api, windows, w, p, heads, mode, seed, scale=qscale, lse=True)
+
+
 def test_errors(api):
     q, k, v = synth.qkv(1, 64, 1, 32, 1, device="cuda")
     with pytest.raises(api.MfError):
