@@ -25,6 +25,8 @@
 
 #include <cuda_bf16.h>
 
+#include <atomic>
+
 namespace mf {
 
 constexpr int kD = 64;                 // head_dim
@@ -434,10 +436,14 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
     if (grid > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MF_CUDA_OK(cudaFuncSetAttribute(window_attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
+    {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
+        static std::atomic<bool> attr_set[64];
+        int dev = 0;
+        MF_CUDA_OK(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
+            MF_CUDA_OK(cudaFuncSetAttribute(window_attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
+        }
     }
     window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(mq, mk, mv,
                                                                                                               prm);

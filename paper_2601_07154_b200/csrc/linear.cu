@@ -16,6 +16,8 @@
 
 #include <cuda_bf16.h>
 
+#include <atomic>
+
 namespace mf {
 
 constexpr int kGM = 128, kGN = 256, kGK = 64, kGStages = 4;
@@ -344,10 +346,14 @@ extern "C" mf_status mf_linear(const void* x, const void* w, const float* bias, 
     if (tiles > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_linear: too many tiles");
     const int grid = static_cast<int>(tiles < sm_count() ? tiles : sm_count());
     const int smem = static_cast<int>(sizeof(GemmSmem)) + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MF_CUDA_OK(cudaFuncSetAttribute(linear_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
+    {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
+        static std::atomic<bool> attr_set[64];
+        int dev = 0;
+        MF_CUDA_OK(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
+            MF_CUDA_OK(cudaFuncSetAttribute(linear_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
+        }
     }
     linear_kernel<<<grid, kGThreads, smem, static_cast<cudaStream_t>(stream)>>>(mx, mw, prm);
     MF_CUDA_OK(cudaGetLastError());
