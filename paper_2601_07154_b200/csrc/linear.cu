@@ -1,13 +1,17 @@
 // mf_linear: out = act(x w^T + bias) (+ residual), bf16 in / fp32 accumulate / bf16 out, for sm_100a
 // (the QKV projection, output projection and MLP around the window attention; reading E1-E4).
 //
-// Persistent kernel, one CTA per SM, 320 threads:
-//   warp 0     TMA producer: x tile (128 rows x 64 k) and w tile (256 rows x 64 k), SWIZZLE_128B, 4-stage ring
-//   warp 1     tcgen05.mma issuer (one thread): D[128 x 256] += x_tile w_tile^T, 4 MMAs of K=16 per stage,
-//              accumulator in TMEM, two accumulators (2 x 256 columns) so the epilogue of tile i overlaps the
-//              main loop of tile i+1
-//   warps 2-9  epilogue: tcgen05.ld 32 columns at a time (TMEM lane = output row; two warps per lane quarter, half
-//              of the columns each), + bias, GELU, + residual, round to bf16, 64 B per thread and chunk to global
+// Persistent kernel, 320 threads per CTA, one CTA per SM, CTAs working in PAIRS (cluster of 2, tcgen05 cta_group::2) on
+// 256 x 256 output tiles (a 1-CTA 128 x 256 instantiation remains for single-band problems and MF_LINEAR_CTAS=1):
+//   warp 0     TMA producer: this CTA's 128 rows of x and its HALF of the w tile (128 output columns) per 64-wide k step,
+//              SWIZZLE_128B, 6-stage ring (32 KB per stage); both CTAs' loads complete on the leader's mbarrier
+//   warp 1     leader CTA only: one thread issues tcgen05.mma.cta_group::2, M = 256, N = 256, 4 x K=16 per stage; the MMA
+//              reads both CTAs' shared memory and accumulates rows 0-127 in the leader's TMEM, 128-255 in the peer's;
+//              tcgen05.commit ... multicast::cluster frees the stage / publishes the accumulator in both CTAs.  Two
+//              accumulators (2 x 256 columns) so the epilogue of tile i overlaps the main loop of tile i+1
+//   warps 2-9  epilogue (both CTAs, own 128 rows): tcgen05.ld 64 columns per pass (TMEM lane = output row; two warps per
+//              lane quarter, half of the columns each), + bias, GELU, + residual, round to bf16, staged through a swizzled
+//              per-warp buffer so that global stores and residual loads are 4 rows x 128 B per warp instruction
 // Output tiles are visited n-fastest, so the CTAs running together share one band of x rows in L2 while w (a few
 // MB) stays L2-resident.  Columns may be split over up to three output tensors (q | k | v): n_split columns each.
 #include "common.h"
@@ -17,18 +21,26 @@
 #include <cuda_bf16.h>
 
 #include <atomic>
+#include <cstdlib>
 
 namespace mf {
 
-constexpr int kGM = 128, kGN = 256, kGK = 64, kGStages = 4;
+constexpr int kGM = 128, kGN = 256, kGK = 64;
 constexpr int kEpiWarps = 8;               // two per TMEM lane quarter: each takes half of the tile's 256 columns
 constexpr int kGThreads = (2 + kEpiWarps) * 32;
 constexpr int kATile = kGM * kGK * 2;      // 16 KB
-constexpr int kBTile = kGN * kGK * 2;      // 32 KB
 
+// kCtas = 1: one CTA per 128 x 256 output tile.  kCtas = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) per 256 x 256
+// tile: each CTA holds its 128 rows of x and HALF of the w tile (128 of the 256 output columns), the leader issues
+// M = 256 MMAs that read both CTAs' shared memory and accumulate into both CTAs' TMEM.  A stage is 32 KB instead of
+// 48 KB, so the same shared memory holds 6 stages: the ring covers 3072 instead of 2048 tensor clocks of load latency.
+template <int kCtas>
 struct GemmSmem {
-    alignas(1024) uint8_t a[kGStages][kATile];
-    alignas(1024) uint8_t b[kGStages][kBTile];
+    static constexpr int kStages = kCtas == 2 ? 6 : 4;
+    static constexpr int kBTile = (kGN / kCtas) * kGK * 2;      // 32 KB, or 16 KB per CTA of a pair
+    static constexpr int kGStages = kStages;
+    alignas(1024) uint8_t a[kStages][kATile];
+    alignas(1024) uint8_t b[kStages][kBTile];
     alignas(16) uint8_t stage[kEpiWarps][32 * 128];      // per epilogue warp: 32 rows x 64 bf16, XOR-swizzled 16-byte chunks
     alignas(8) uint64_t full[kGStages];
     uint64_t empty[kGStages], acc_full[2], acc_empty[2];
@@ -37,7 +49,7 @@ struct GemmSmem {
 
 struct GemmParams {
     int M, N, K, n_split;
-    int m_tiles, n_tiles;
+    int m_tiles, n_tiles;       // m_tiles counts 128-row (kCtas = 1) or 256-row (kCtas = 2) bands
     const float* bias;
     const __nv_bfloat16* residual;
     __nv_bfloat16* out[3];
@@ -45,6 +57,7 @@ struct GemmParams {
 };
 
 constexpr uint32_t kIdescGemm = ptx::idesc_bf16_f32(kGM, kGN, 0, 0);
+constexpr uint32_t kIdescGemmPair = ptx::idesc_bf16_f32(2 * kGM, kGN, 0, 0);
 
 // Reading E3 (exact erf GELU).  erf by Abramowitz & Stegun 7.1.26 (|error| <= 1.5e-7, far below the bf16 output's 2^-9):
 // erf(x) = 1 - (a1 t + ... + a5 t^5) exp(-x^2), t = 1 / (1 + p x), x >= 0; odd in x.
@@ -67,13 +80,19 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
                  : "memory");
 }
 
+template <int kCtas>
 __global__ void __launch_bounds__(kGThreads, 1)
 linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__ CUtensorMap map_w, const GemmParams prm) {
+    using Smem = GemmSmem<kCtas>;
+    constexpr int kGStages = Smem::kStages;
+    constexpr int kBTile = Smem::kBTile;
     extern __shared__ uint8_t smem_raw[];
-    GemmSmem& sm = *reinterpret_cast<GemmSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_tiles_total = prm.m_tiles * prm.n_tiles;
     const int k_steps = prm.K / kGK;
+    const int rank = kCtas == 2 ? static_cast<int>(ptx::cluster_ctarank()) : 0;     // 0 = leader of the pair
+    const int tile0 = blockIdx.x / kCtas, tile_step = gridDim.x / kCtas;
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&map_x);
@@ -84,13 +103,17 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(&sm.acc_full[b], 1);
-            ptx::mbar_init(&sm.acc_empty[b], kEpiWarps);   // one arrival per epilogue warp
+            ptx::mbar_init(&sm.acc_empty[b], kEpiWarps * kCtas);   // one arrival per epilogue warp (of both CTAs of a pair)
         }
         ptx::fence_barrier_init();
     }
-    if (warp == 1) ptx::tmem_alloc(&sm.tmem_base, 512);
+    if (warp == 1) {
+        if (kCtas == 2) ptx::tmem_alloc_pair(&sm.tmem_base, 512);
+        else ptx::tmem_alloc(&sm.tmem_base, 512);
+    }
     ptx::tc_fence_before();
-    __syncthreads();
+    if (kCtas == 2) ptx::cluster_sync();
+    else __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
 
@@ -98,22 +121,32 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         // ===================== TMA producer =====================
         if (lane == 0) {
             int it = 0;
-            for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x) {
+            for (int tile = tile0; tile < n_tiles_total; tile += tile_step) {
                 const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
                 for (int ks = 0; ks < k_steps; ++ks, ++it) {
                     const int st = it % kGStages;
                     ptx::mbar_wait(&sm.empty[st], ((it / kGStages) & 1) ^ 1);
-                    ptx::mbar_arrive_expect_tx(&sm.full[st], kATile + kBTile);
-                    tma_load_2d(sm.a[st], &map_x, &sm.full[st], ks * kGK, mt * kGM);
-                    tma_load_2d(sm.b[st], &map_w, &sm.full[st], ks * kGK, nt * kGN);
+                    if (kCtas == 1) {
+                        ptx::mbar_arrive_expect_tx(&sm.full[st], kATile + kBTile);
+                        tma_load_2d(sm.a[st], &map_x, &sm.full[st], ks * kGK, mt * kGM);
+                        tma_load_2d(sm.b[st], &map_w, &sm.full[st], ks * kGK, nt * kGN);
+                    } else {
+                        // Both CTAs' loads complete on the LEADER's barrier (the MMA issuer waits there): the leader arrives
+                        // once expecting the bytes of both, the peer only contributes bytes.  The peer cannot run a phase
+                        // ahead: it refills a stage only after the leader's MMAs on it have completed (multicast commit).
+                        const uint32_t lead_full = ptx::mapa(&sm.full[st], 0);
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(&sm.full[st], 2 * (kATile + kBTile));
+                        ptx::tma_load_2d_pair(sm.a[st], &map_x, lead_full, ks * kGK, mt * (2 * kGM) + rank * kGM);
+                        ptx::tma_load_2d_pair(sm.b[st], &map_w, lead_full, ks * kGK, nt * kGN + rank * (kGN / 2));
+                    }
                 }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        if (lane == 0) {
+        if (lane == 0 && rank == 0) {
             int it = 0, local = 0;
-            for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x, ++local) {
+            for (int tile = tile0; tile < n_tiles_total; tile += tile_step, ++local) {
                 const int buf = local & 1;
                 ptx::mbar_wait(&sm.acc_empty[buf], ((local >> 1) & 1) ^ 1);     // epilogue has drained this accumulator
                 ptx::tc_fence_after();
@@ -125,10 +158,15 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                     const uint64_t ad = ptx::smem_desc_sw128(ptx::smem_u32(sm.a[st]));
                     const uint64_t bd = ptx::smem_desc_sw128(ptx::smem_u32(sm.b[st]));
 #pragma unroll
-                    for (int i = 0; i < kGK / 16; ++i) ptx::mma_ss(d, ad + 2 * i, bd + 2 * i, kIdescGemm, (ks > 0 || i > 0) ? 1u : 0u);
-                    ptx::mma_commit(&sm.empty[st]);
+                    for (int i = 0; i < kGK / 16; ++i) {
+                        if (kCtas == 2) ptx::mma_ss_pair(d, ad + 2 * i, bd + 2 * i, kIdescGemmPair, (ks > 0 || i > 0) ? 1u : 0u);
+                        else ptx::mma_ss(d, ad + 2 * i, bd + 2 * i, kIdescGemm, (ks > 0 || i > 0) ? 1u : 0u);
+                    }
+                    if (kCtas == 2) ptx::mma_commit_pair(&sm.empty[st], 3);        // frees the stage in both CTAs
+                    else ptx::mma_commit(&sm.empty[st]);
                 }
-                ptx::mma_commit(&sm.acc_full[buf]);
+                if (kCtas == 2) ptx::mma_commit_pair(&sm.acc_full[buf], 3);
+                else ptx::mma_commit(&sm.acc_full[buf]);
             }
         }
     } else {
@@ -143,10 +181,10 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         uint4* stage = reinterpret_cast<uint4*>(sm.stage[warp - 2]);      // [32 rows][8 chunks of 16 B]
         const int crow = lane >> 3, cchunk = lane & 7;     // coalesced phase: this lane's row (of 4) and 16-byte chunk
         int local = 0;
-        for (int tile = blockIdx.x; tile < n_tiles_total; tile += gridDim.x, ++local) {
+        for (int tile = tile0; tile < n_tiles_total; tile += tile_step, ++local) {
             const int buf = local & 1;
             const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
-            const int row0 = mt * kGM + quarter * 32;      // first of this warp's 32 rows
+            const int row0 = mt * (kCtas * kGM) + rank * kGM + quarter * 32;      // first of this warp's 32 rows
             const int n0 = nt * kGN + 128 * chalf;         // first of this warp's 128 columns
             const int which = n0 / prm.n_split, c0 = n0 - which * prm.n_split;
             __nv_bfloat16* dst = prm.out[which] + c0;
@@ -184,7 +222,10 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                 if (g == 1) {                              // the accumulator is in registers: hand it back to the MMA issuer
                     ptx::tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&sm.acc_empty[buf]);
+                    if (lane == 0) {
+                        if (kCtas == 2 && rank != 0) ptx::mbar_arrive_cluster(ptx::mapa(&sm.acc_empty[buf], 0));
+                        else ptx::mbar_arrive(&sm.acc_empty[buf]);
+                    }
                 }
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {              // 8 columns per step
@@ -229,8 +270,12 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         }
     }
     ptx::tc_fence_before();
-    __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+    if (kCtas == 2) ptx::cluster_sync();                   // the peer may still be arriving on this CTA's barriers / reading TMEM
+    else __syncthreads();
+    if (warp == 1) {
+        if (kCtas == 2) ptx::tmem_dealloc_pair(tmem, 512);
+        else ptx::tmem_dealloc(tmem, 512);
+    }
 }
 
 }  // namespace mf
@@ -310,6 +355,23 @@ static mf_status make_map_2d(CUtensorMap* map, const void* base, long long rows,
 
 }  // namespace mf
 
+namespace mf {
+// the opt-in shared-memory size is a per-device attribute of each kernel instantiation: set it once per device
+template <typename K>
+static cudaError_t ensure_smem(K kernel, int smem, int slot) {
+    static std::atomic<bool> done[2][64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !done[slot][dev].load(std::memory_order_acquire)) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) done[slot][dev].store(true, std::memory_order_release);
+    }
+    return cudaSuccess;
+}
+}  // namespace mf
+
 extern "C" mf_status mf_linear(const void* x, const void* w, const float* bias, const void* residual, void* out0,
                                void* out1, void* out2, int M, int N, int K, int n_split, mf_activation act,
                                void* stream) {
@@ -330,11 +392,14 @@ extern "C" mf_status mf_linear(const void* x, const void* w, const float* bias, 
     mf_status st = require_sm100();
     if (st != MF_OK) return st;
     CUtensorMap mx, mw;
+    // CTA pairs (256 x 256 tiles) unless the problem is a single 128-row band or MF_LINEAR_CTAS=1 asks for the 1-CTA kernel
+    static const int forced = [] { const char* e = getenv("MF_LINEAR_CTAS"); return e ? atoi(e) : 0; }();
+    const int ctas = forced == 1 ? 1 : (forced == 2 ? 2 : (M > kGM ? 2 : 1));
     if ((st = make_map_2d(&mx, x, M, K, kGM)) != MF_OK) return st;
-    if ((st = make_map_2d(&mw, w, N, K, kGN)) != MF_OK) return st;
+    if ((st = make_map_2d(&mw, w, N, K, kGN / ctas)) != MF_OK) return st;
     GemmParams prm;
     prm.M = M; prm.N = N; prm.K = K; prm.n_split = n_split;
-    prm.m_tiles = (M + kGM - 1) / kGM;
+    prm.m_tiles = (M + ctas * kGM - 1) / (ctas * kGM);
     prm.n_tiles = N / kGN;
     prm.bias = bias;
     prm.residual = static_cast<const __nv_bfloat16*>(residual);
@@ -344,18 +409,30 @@ extern "C" mf_status mf_linear(const void* x, const void* w, const float* bias, 
     prm.act = act;
     const long long tiles = static_cast<long long>(prm.m_tiles) * prm.n_tiles;
     if (tiles > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_linear: too many tiles");
-    const int grid = static_cast<int>(tiles < sm_count() ? tiles : sm_count());
-    const int smem = static_cast<int>(sizeof(GemmSmem)) + 1024;
-    {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
-        static std::atomic<bool> attr_set[64];
-        int dev = 0;
-        MF_CUDA_OK(cudaGetDevice(&dev));
-        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
-            MF_CUDA_OK(cudaFuncSetAttribute(linear_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
-        }
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    if (ctas == 1) {
+        const int grid = static_cast<int>(tiles < sm_count() ? tiles : sm_count());
+        const int smem = static_cast<int>(sizeof(GemmSmem<1>)) + 1024;
+        MF_CUDA_OK(ensure_smem(linear_kernel<1>, smem, 0));
+        linear_kernel<1><<<grid, kGThreads, smem, cs>>>(mx, mw, prm);
+    } else {
+        const int pairs = static_cast<int>(tiles < sm_count() / 2 ? tiles : sm_count() / 2);
+        const int smem = static_cast<int>(sizeof(GemmSmem<2>)) + 1024;
+        MF_CUDA_OK(ensure_smem(linear_kernel<2>, smem, 1));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(2 * pairs);
+        cfg.blockDim = dim3(kGThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = cs;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        MF_CUDA_OK(cudaLaunchKernelEx(&cfg, linear_kernel<2>, mx, mw, prm));
     }
-    linear_kernel<<<grid, kGThreads, smem, static_cast<cudaStream_t>(stream)>>>(mx, mw, prm);
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
 }
