@@ -46,3 +46,31 @@ def brute_force_pixel(points, x, y):
     import math
     return sum(math.exp(-(((x - float(u)) ** 2) + ((y - float(v)) ** 2)) / (2.0 * float(s) * float(s)))
                for (u, v, s) in points)
+
+
+def upsample_bilinear(depth_lo, width, height):
+    """Reading F1 (the paper is silent on how the model-resolution depth reaches the focus-map
+    resolution, B7/D4): bilinear interpolation with half-pixel centres and edge clamping, i.e. what
+    torch.nn.functional.interpolate(mode="bilinear", align_corners=False) computes.  For output column x of `width`
+    from an input row of w_lo samples: src = max(0, (x + 1/2) w_lo / width - 1/2), x0 = floor(src),
+    x1 = min(x0 + 1, w_lo - 1), lambda = src - x0; the same along y; D = (1-ly)((1-lx) d00 + lx d01) + ly((1-lx) d10 + lx d11).
+    depth_lo [h_lo, w_lo] -> fp64 [height, width].  Plain loops over the output axes, no library interpolation."""
+    d = np.asarray(depth_lo, dtype=np.float64)
+    h_lo, w_lo = d.shape
+
+    def taps(n_out, n_in):
+        i0, i1, lam = [], [], []
+        for o in range(n_out):
+            src = max(0.0, (o + 0.5) * n_in / n_out - 0.5)
+            a = int(np.floor(src))
+            a = min(a, n_in - 1)
+            i0.append(a)
+            i1.append(min(a + 1, n_in - 1))
+            lam.append(src - a)
+        return np.array(i0), np.array(i1), np.array(lam, dtype=np.float64)
+
+    x0, x1, lx = taps(width, w_lo)
+    y0, y1, ly = taps(height, h_lo)
+    top = d[y0][:, x0] * (1.0 - lx)[None, :] + d[y0][:, x1] * lx[None, :]
+    bot = d[y1][:, x0] * (1.0 - lx)[None, :] + d[y1][:, x1] * lx[None, :]
+    return top * (1.0 - ly)[:, None] + bot * ly[:, None]

@@ -87,3 +87,26 @@ def test_sigma_per_point_is_used():
     pts = _pts((8.0, 8.0, 1.0), (24.0, 8.0, 6.0))
     u_map = orr.unnormalised(pts, 32, 16)
     assert abs(u_map[8, 12] - (math.exp(-16 / 2.0) + math.exp(-144 / 72.0))) < 1e-15
+
+
+def test_upsample_bilinear_pins():
+    import torch
+    rng = np.random.default_rng(3)
+    lo = rng.uniform(1.0, 30.0, (7, 9))
+    for (h, w) in [(14, 18), (20, 31), (7, 9), (5, 4), (33, 64)]:
+        up = orr.upsample_bilinear(lo, w, h)
+        ref = torch.nn.functional.interpolate(torch.from_numpy(lo)[None, None], size=(h, w), mode="bilinear",
+                                              align_corners=False)[0, 0].numpy()
+        assert np.abs(up - ref).max() < 1e-12
+    assert np.array_equal(orr.upsample_bilinear(lo, 9, 7), lo)                       # same size: identity
+    assert np.abs(orr.upsample_bilinear(np.full((3, 5), 4.25), 40, 24) - 4.25).max() < 1e-15   # constants are kept
+    # a linear ramp is reproduced exactly away from the clamped border: D(x) = a (x + 1/2) w_lo / W - a/2
+    ramp = np.tile(np.arange(6, dtype=np.float64) * 2.0, (4, 1))
+    up = orr.upsample_bilinear(ramp, 24, 4)
+    x = np.arange(24)
+    src = np.clip((x + 0.5) * 6 / 24 - 0.5, 0.0, 5.0)
+    assert np.abs(up[0] - 2.0 * src).max() < 1e-13
+    # 2x upscale of two samples (hand values): src = -0.25 -> 0, 0.25, 0.75, 1.25 -> clamped to sample 1
+    assert np.allclose(orr.upsample_bilinear(np.array([[0.0, 8.0]]), 4, 1), [[0.0, 2.0, 6.0, 8.0]], atol=1e-15)
+    # a transposed call must differ (rows and columns are not interchangeable)
+    assert orr.upsample_bilinear(lo, 18, 14).shape == (14, 18)
