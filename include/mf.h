@@ -148,6 +148,20 @@ mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_fra
                           int32_t* focus_index, void* workspace, size_t workspace_bytes,
                           void* stream);
 
+/* mf_motion_focus with the depth at the MODEL's resolution (the paper does not say how its depth
+ * maps reach the focus-map resolution, reading F1 in DESIGN.md): depth_lowres is fp32 [count, depth_height, depth_width]
+ * and is interpolated inside the render pass, bilinear with half-pixel centres and edge clamping (what
+ * torch.nn.functional.interpolate(mode="bilinear", align_corners=False) computes), so the full-resolution depth never
+ * exists in HBM: the pass writes 8 B/pixel and reads almost nothing.  focus_map and guided_depth are required; every other
+ * argument as in mf_motion_focus (same workspace size).
+ */
+mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intrinsics K, int num_frames,
+                                    int render_begin, int render_end, int width, int height,
+                                    const float* depth_lowres, int depth_width, int depth_height,
+                                    const mf_focus_params* params, float* focus_map, float* guided_depth,
+                                    float* focus_uv, int32_t* focus_index, void* workspace,
+                                    size_t workspace_bytes, void* stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Host-buffer conveniences (end-to-end path): same semantics, every pointer is HOST memory
  * (pinned memory makes the copies asynchronous).  They allocate device buffers, copy in,

@@ -20,7 +20,7 @@ ACT_NONE, ACT_GELU = 0, 1
 EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
            "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
-           "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step"]
+           "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step", "mf_motion_focus_upsampled"]
 
 
 class MfError(RuntimeError):
@@ -75,6 +75,8 @@ def lib():
         L.mf_block_forward.argtypes = [vp, ctypes.POINTER(BlockWeights), vp, ci, ci, ci, ci, ci, ci, ci, cf, vp, ctypes.c_size_t, vp]
         L.mf_chain_state_size.restype = ctypes.c_size_t
         L.mf_chain_poses_step.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
+        L.mf_motion_focus_upsampled.argtypes = [vp, Intrinsics, ci, ci, ci, ci, ci, vp, ci, ci, ctypes.POINTER(FocusParams),
+                                                vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
         _lib = L
     return _lib
 
@@ -176,6 +178,38 @@ def motion_focus(global_w2c, fx, fy, cx, cy, width, height, params=None, depth=N
                                  _ptr(uv), _ptr(idx), _ptr(workspace), workspace.numel(), _stream()))
     return {"focus_map": fmap, "guided_depth": guided, "focus_uv": uv, "focus_index": idx,
             "workspace": workspace}
+
+
+def motion_focus_upsampled(global_w2c, fx, fy, cx, cy, width, height, depth_lowres, params=None, render_begin=0,
+                           render_end=None, workspace=None, out=None):
+    """mf_motion_focus_upsampled: depth_lowres fp32 CUDA [count, h_lo, w_lo] is interpolated (bilinear, half-pixel centres)
+    to width x height inside the render pass.  Returns dict(focus_map, guided_depth, focus_uv, focus_index)."""
+    _dev(global_w2c, torch.float64, "global_w2c")
+    _dev(depth_lowres, torch.float32, "depth_lowres")
+    n = global_w2c.shape[0]
+    render_end = n if render_end is None else render_end
+    count = render_end - render_begin
+    if depth_lowres.dim() != 3 or depth_lowres.shape[0] != count:
+        raise MfError("depth_lowres must be [count, h_lo, w_lo]")
+    params = focus_params() if params is None else params
+    dev = global_w2c.device
+    out = {} if out is None else out
+    fmap = out.get("focus_map")
+    if fmap is None:
+        fmap = torch.empty((count, height, width), device=dev, dtype=torch.float32)
+    guided = out.get("guided_depth")
+    if guided is None:
+        guided = torch.empty((count, height, width), device=dev, dtype=torch.float32)
+    uv = torch.empty((count, 2), device=dev, dtype=torch.float32)
+    idx = torch.empty((count,), device=dev, dtype=torch.int32)
+    need = lib().mf_motion_focus_workspace_size(count, width, height, params.n_points)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty((max(need, 16),), device=dev, dtype=torch.uint8)
+    _check(lib().mf_motion_focus_upsampled(_ptr(global_w2c), Intrinsics(fx, fy, cx, cy), n, render_begin, render_end, width,
+                                           height, _ptr(depth_lowres), depth_lowres.shape[2], depth_lowres.shape[1],
+                                           ctypes.byref(params), _ptr(fmap), _ptr(guided), _ptr(uv), _ptr(idx), _ptr(workspace),
+                                           workspace.numel(), _stream()))
+    return {"focus_map": fmap, "guided_depth": guided, "focus_uv": uv, "focus_index": idx, "workspace": workspace}
 
 
 # ---- host-buffer entry points (end-to-end path) ---------------------------------------------------

@@ -578,14 +578,14 @@ __device__ __forceinline__ void st_stream(float4* p, float4 v) {
 }
 
 // rows [ya, yb) of this thread's 4 columns where the map is identically zero: M = 0, G = 0 * D (depth is still read)
-template <bool HAS_DEPTH, bool HAS_G>
+template <bool HAS_DEPTH, bool HAS_G, bool LOWRES>
 __device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth, float* __restrict__ focus_map,
                                                  float* __restrict__ guided, size_t img, int width, int ya, int yb) {
     constexpr int U = 8;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int y = ya; y < yb; y += U) {
         float4 d[U];
-        if (HAS_G) {
+        if (HAS_G && !LOWRES) {
 #pragma unroll
             for (int r = 0; r < U; ++r)
                 if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
@@ -595,20 +595,34 @@ __device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth
             if (y + r < yb) {
                 const size_t o = img + static_cast<size_t>(y + r) * width;
                 st_stream(reinterpret_cast<float4*>(focus_map + o), zero);
-                if (HAS_G)
+                if (HAS_G)          // LOWRES: the interpolated depth is finite wherever its samples are, 0 * D = 0 is not read back
                     st_stream(reinterpret_cast<float4*>(guided + o),
-                              make_float4(0.f * d[r].x, 0.f * d[r].y, 0.f * d[r].z, 0.f * d[r].w));
+                              LOWRES ? zero : make_float4(0.f * d[r].x, 0.f * d[r].y, 0.f * d[r].z, 0.f * d[r].w));
             }
         }
     }
 }
 
-template <int NP, bool HAS_DEPTH, bool HAS_G>
+// Bilinear taps of reading F1 (half-pixel centres, edge clamp) for output index o of n_out from n_in samples, in exact
+// integer arithmetic: src = max(0, ((2o+1) n_in - n_out) / (2 n_out)).
+__device__ __forceinline__ void bilinear_taps(int o, int n_out, int n_in, int& i0, int& i1, float& lam) {
+    const long long num = static_cast<long long>(2 * o + 1) * n_in - n_out;
+    if (num <= 0) {
+        i0 = 0;
+        lam = 0.f;
+    } else {
+        i0 = min(static_cast<int>(num / (2 * n_out)), n_in - 1);
+        lam = static_cast<float>(num - static_cast<long long>(i0) * 2 * n_out) / static_cast<float>(2 * n_out);
+    }
+    i1 = min(i0 + 1, n_in - 1);
+}
+
+template <int NP, bool HAS_DEPTH, bool HAS_G, bool LOWRES>
 __global__ void __launch_bounds__(kRenderThreads, MF_RENDER_MINB)
 render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const FrameMeta* __restrict__ meta,
               const uint32_t* __restrict__ colmask, const uint32_t* __restrict__ rowmask,
               const float* __restrict__ depth, float* __restrict__ focus_map, float* __restrict__ guided,
-              int width, int height, int blocks_per_frame, int norm) {
+              int width, int height, int blocks_per_frame, int norm, int dw, int dh) {
     pdl_wait();                             // norm_kernel's (and, through it, tables_kernel's) output
     const int f = blockIdx.x / blocks_per_frame;
     const int b = blockIdx.x - f * blocks_per_frame;
@@ -639,7 +653,7 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
                    __ldg(rowmask + static_cast<size_t>(f) * tr + rb);
     pts_live = __reduce_or_sync(0xffffffffu, pts_live);
     const int ya = pts_live ? y0 : y1, yb = y1;                  // rows computed by this thread: [ya, yb)
-    stream_zero_rows<HAS_DEPTH, HAS_G>(depth, focus_map, guided, img, width, y0, ya);
+    stream_zero_rows<HAS_DEPTH, HAS_G, LOWRES>(depth, focus_map, guided, img, width, y0, ya);
     if (pts_live) {
         float4 e[NP];
         const float* exf = ex + static_cast<size_t>(f) * NP * width + x;
@@ -666,12 +680,42 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
             __syncwarp();
         }
         constexpr int U = MF_RENDER_U;
+        // LOWRES: depth is [count, dh, dw] at the model's resolution and is interpolated here (reading F1); the four
+        // columns' taps are fixed for the thread, the row taps change per row.  The samples come from L1/L2.
+        int tx0[4] = {0, 0, 0, 0}, tx1[4] = {0, 0, 0, 0};
+        float tlx[4] = {0.f, 0.f, 0.f, 0.f};
+        const float* dlo = depth;
+        if (LOWRES) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) bilinear_taps(x + c, width, dw, tx0[c], tx1[c], tlx[c]);
+            dlo = depth + static_cast<size_t>(f) * dh * dw;
+        }
         for (int y = ya; y < yb; y += U) {
             float4 d[U];
-            if (HAS_DEPTH) {
+            if (HAS_DEPTH && !LOWRES) {
 #pragma unroll
                 for (int r = 0; r < U; ++r)
                     if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
+            }
+            if (LOWRES) {
+#pragma unroll
+                for (int r = 0; r < U; ++r) {
+                    if (y + r < yb) {
+                        int ty0, ty1;
+                        float ly;
+                        bilinear_taps(y + r, height, dh, ty0, ty1, ly);
+                        const float* r0 = dlo + static_cast<size_t>(ty0) * dw;
+                        const float* r1 = dlo + static_cast<size_t>(ty1) * dw;
+                        float v[4];
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            const float top = fmaf(tlx[c], __ldg(r0 + tx1[c]) - __ldg(r0 + tx0[c]), __ldg(r0 + tx0[c]));
+                            const float bot = fmaf(tlx[c], __ldg(r1 + tx1[c]) - __ldg(r1 + tx0[c]), __ldg(r1 + tx0[c]));
+                            v[c] = fmaf(ly, bot - top, top);
+                        }
+                        d[r] = make_float4(v[0], v[1], v[2], v[3]);
+                    }
+                }
             }
 #pragma unroll
             for (int r = 0; r < U; ++r) {
@@ -705,22 +749,26 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
 
 template <int NP>
 static void launch_render(const Workspace& ws, const float* depth, float* focus_map, float* guided, int count,
-                          int width, int height, int norm, cudaStream_t stream) {
+                          int width, int height, int norm, int dw, int dh, cudaStream_t stream) {
     const int row_blocks = (height + kRowsPerThread - 1) / kRowsPerThread;
     const long long threads = static_cast<long long>(width / 4) * row_blocks;
     const int bpf = static_cast<int>((threads + kRenderThreads - 1) / kRenderThreads);
     const unsigned grid = static_cast<unsigned>(bpf) * static_cast<unsigned>(count);
     const size_t smem = sizeof(float) * (kRenderThreads / 32) * kStageRows * NP;
     if (smem > 48 * 1024) {
-        cudaFuncSetAttribute(render_kernel<NP, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-        cudaFuncSetAttribute(render_kernel<NP, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        cudaFuncSetAttribute(render_kernel<NP, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        cudaFuncSetAttribute(render_kernel<NP, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        cudaFuncSetAttribute(render_kernel<NP, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     }
-    if (guided)
-        launch_pdl(render_kernel<NP, true, true>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
-                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm);
+    if (guided && dw > 0)
+        launch_pdl(render_kernel<NP, true, true, true>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
+                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm, dw, dh);
+    else if (guided)
+        launch_pdl(render_kernel<NP, true, true, false>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
+                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm, 0, 0);
     else
-        launch_pdl(render_kernel<NP, false, false>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt, ws.meta,
-                   ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm);
+        launch_pdl(render_kernel<NP, false, false, false>, dim3(grid), dim3(kRenderThreads), smem, stream, ws.ex, ws.eyt,
+                   ws.meta, ws.colmask, ws.rowmask, depth, focus_map, guided, width, height, bpf, norm, 0, 0);
 }
 
 }  // namespace mf
@@ -730,11 +778,11 @@ extern "C" size_t mf_motion_focus_workspace_size(int count, int width, int heigh
     return mf::carve(nullptr, count, width, height, n_points, nullptr);
 }
 
-extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_frames, int render_begin,
-                                     int render_end, int width, int height, const float* depth,
-                                     const mf_focus_params* params, float* focus_map, float* guided_depth,
-                                     float* focus_uv, int32_t* focus_index, void* workspace, size_t workspace_bytes,
-                                     void* stream) {
+// depth_width == 0: depth is [count, height, width]; otherwise [count, depth_height, depth_width], interpolated (reading F1)
+static mf_status motion_focus_impl(const double* global_w2c, mf_intrinsics K, int num_frames, int render_begin, int render_end,
+                                   int width, int height, const float* depth, int depth_width, int depth_height,
+                                   const mf_focus_params* params, float* focus_map, float* guided_depth, float* focus_uv,
+                                   int32_t* focus_index, void* workspace, size_t workspace_bytes, void* stream) {
     using namespace mf;
     if (!global_w2c || !params) return fail(MF_ERR_INVALID_ARG, "mf_motion_focus: NULL poses or params");
     if (num_frames < 1 || render_begin < 0 || render_end > num_frames || render_end <= render_begin)
@@ -811,14 +859,14 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
         w.eyt = ws.eyt + static_cast<size_t>(f0) * height * npad;
         w.colmask = ws.colmask + static_cast<size_t>(f0) * tc;
         w.rowmask = ws.rowmask + static_cast<size_t>(f0) * tr;
-        const float* d = depth ? depth + f0 * img : nullptr;
+        const float* d = depth ? depth + f0 * (depth_width > 0 ? static_cast<size_t>(depth_width) * depth_height : img) : nullptr;
         float* m = focus_map + f0 * img;
         float* gd = guided_depth ? guided_depth + f0 * img : nullptr;
         switch (npad) {
-            case 8: launch_render<8>(w, d, m, gd, n, width, height, params->norm, q); break;
-            case 16: launch_render<16>(w, d, m, gd, n, width, height, params->norm, q); break;
-            case 24: launch_render<24>(w, d, m, gd, n, width, height, params->norm, q); break;
-            default: launch_render<32>(w, d, m, gd, n, width, height, params->norm, q); break;
+            case 8: launch_render<8>(w, d, m, gd, n, width, height, params->norm, depth_width, depth_height, q); break;
+            case 16: launch_render<16>(w, d, m, gd, n, width, height, params->norm, depth_width, depth_height, q); break;
+            case 24: launch_render<24>(w, d, m, gd, n, width, height, params->norm, depth_width, depth_height, q); break;
+            default: launch_render<32>(w, d, m, gd, n, width, height, params->norm, depth_width, depth_height, q); break;
         }
         return cudaGetLastError();
     };
@@ -826,4 +874,26 @@ extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, 
     MF_CUDA_OK(prepare(0, count, s));
     if (focus_map) MF_CUDA_OK(render(0, count, s));
     return MF_OK;
+}
+
+extern "C" mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_frames, int render_begin,
+                                     int render_end, int width, int height, const float* depth,
+                                     const mf_focus_params* params, float* focus_map, float* guided_depth,
+                                     float* focus_uv, int32_t* focus_index, void* workspace, size_t workspace_bytes,
+                                     void* stream) {
+    return motion_focus_impl(global_w2c, K, num_frames, render_begin, render_end, width, height, depth, 0, 0, params, focus_map,
+                             guided_depth, focus_uv, focus_index, workspace, workspace_bytes, stream);
+}
+
+extern "C" mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intrinsics K, int num_frames, int render_begin,
+                                               int render_end, int width, int height, const float* depth_lowres,
+                                               int depth_width, int depth_height, const mf_focus_params* params,
+                                               float* focus_map, float* guided_depth, float* focus_uv, int32_t* focus_index,
+                                               void* workspace, size_t workspace_bytes, void* stream) {
+    if (!depth_lowres || !guided_depth || !focus_map)
+        return mf::fail(MF_ERR_INVALID_ARG, "mf_motion_focus_upsampled: depth_lowres, focus_map and guided_depth are required");
+    if (depth_width < 1 || depth_height < 1)
+        return mf::fail(MF_ERR_INVALID_ARG, "mf_motion_focus_upsampled: bad depth size %dx%d", depth_width, depth_height);
+    return motion_focus_impl(global_w2c, K, num_frames, render_begin, render_end, width, height, depth_lowres, depth_width,
+                             depth_height, params, focus_map, guided_depth, focus_uv, focus_index, workspace, workspace_bytes, stream);
 }

@@ -199,6 +199,30 @@ def test_focus_chain_to_focus_pipeline_bit_exact_index(api):
     assert np.array_equal(uv[2:].view(np.uint32), ref[2:].view(np.uint32))
 
 
+@pytest.mark.parametrize("cfg_idx,n_frames,rb,re_,lo", [(0, 6, 0, 6, (16, 16)), (1, 24, 16, 24, (294, 518)), (3, 22, 19, 22, (294, 518))])
+def test_focus_with_upsampled_depth(api, cfg_idx, n_frames, rb, re_, lo):
+    # NEXT-4, reading F1: depth at the model's resolution, interpolated inside the render pass
+    cfg = synth.CONFIGS[cfg_idx]
+    w, h = cfg["width"], cfg["height"]
+    poses = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
+    dlo = synth.depth(re_ - rb, lo[0], lo[1], synth.seed_for(cfg_idx, 4)).numpy()
+    prm = api.focus_params(n_points=15, sigma=cfg["sigma"])
+    out = api.motion_focus_upsampled(torch.from_numpy(np.asarray(poses)).cuda(), cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], w, h,
+                                     torch.from_numpy(dlo).cuda(), prm, render_begin=rb, render_end=re_)
+    same = api.motion_focus(torch.from_numpy(np.asarray(poses)).cuda(), cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], w, h, prm,
+                            render_begin=rb, render_end=re_, want_guided=False)
+    torch.cuda.synchronize()
+    assert torch.equal(out["focus_map"], same["focus_map"]) and torch.equal(out["focus_index"], same["focus_index"])
+    frames = op.motion_points(poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], w, h, 15, cfg["sigma"], render_begin=rb, render_end=re_)
+    gd = out["guided_depth"].cpu().numpy()
+    worst = 0.0
+    for f in range(0, re_ - rb, max(1, (re_ - rb) // 3)):
+        up = orr.upsample_bilinear(dlo[f], w, h)
+        _, g = orr.focus_map(frames[f]["points"], w, h, orr.NORM_MAX, up)
+        worst = max(worst, _focus_tolerance(gd[f], g))
+    assert worst <= 1.0, worst
+
+
 def test_focus_degenerate_inputs(api):
     k = (200.0, 200.0, 112.0, 112.0)
     ident = np.tile(np.eye(4), (6, 1, 1))
