@@ -153,7 +153,7 @@ mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_fra
  * and is interpolated inside the render pass, bilinear with half-pixel centres and edge clamping (what
  * torch.nn.functional.interpolate(mode="bilinear", align_corners=False) computes), so the full-resolution depth never
  * exists in HBM: the pass writes 8 B/pixel and reads almost nothing.  focus_map and guided_depth are required; every other
- * argument as in mf_motion_focus (same workspace size).
+ * argument as in mf_motion_focus (same workspace size).  Image and depth sizes above 32767 return MF_ERR_UNSUPPORTED.
  */
 mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intrinsics K, int num_frames,
                                     int render_begin, int render_end, int width, int height,

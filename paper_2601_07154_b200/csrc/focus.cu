@@ -605,20 +605,21 @@ __device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth
 
 // Bilinear taps of reading F1 (half-pixel centres, edge clamp) for output index o of n_out from n_in samples, in exact
 // integer arithmetic: src = max(0, ((2o+1) n_in - n_out) / (2 n_out)).
-__device__ __forceinline__ void bilinear_taps(int o, int n_out, int n_in, int& i0, int& i1, float& lam) {
-    const long long num = static_cast<long long>(2 * o + 1) * n_in - n_out;
+// Sizes are < 2^15 (checked by the caller), so the numerator fits 32 bits; inv_den = 1 / (2 n_out).
+__device__ __forceinline__ void bilinear_taps(int o, int n_out, int n_in, float inv_den, int& i0, int& i1, float& lam) {
+    const int num = (2 * o + 1) * n_in - n_out;
     if (num <= 0) {
         i0 = 0;
         lam = 0.f;
     } else {
-        i0 = min(static_cast<int>(num / (2 * n_out)), n_in - 1);
-        lam = static_cast<float>(num - static_cast<long long>(i0) * 2 * n_out) / static_cast<float>(2 * n_out);
+        i0 = min(num / (2 * n_out), n_in - 1);
+        lam = static_cast<float>(num - i0 * 2 * n_out) * inv_den;
     }
     i1 = min(i0 + 1, n_in - 1);
 }
 
 template <int NP, bool HAS_DEPTH, bool HAS_G, bool LOWRES>
-__global__ void __launch_bounds__(kRenderThreads, MF_RENDER_MINB)
+__global__ void __launch_bounds__(kRenderThreads, LOWRES ? 2 : MF_RENDER_MINB)
 render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const FrameMeta* __restrict__ meta,
               const uint32_t* __restrict__ colmask, const uint32_t* __restrict__ rowmask,
               const float* __restrict__ depth, float* __restrict__ focus_map, float* __restrict__ guided,
@@ -681,41 +682,37 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
         }
         constexpr int U = MF_RENDER_U;
         // LOWRES: depth is [count, dh, dw] at the model's resolution and is interpolated here (reading F1); the four
-        // columns' taps are fixed for the thread, the row taps change per row.  The samples come from L1/L2.
+        // columns' taps are fixed for the thread, the row taps change per row.  One low-res row is interpolated
+        // horizontally to the thread's four columns once (hrow): successive output rows reuse the same two low-res rows
+        // (top, bot) until the row taps move on, so a thread loads each low-res row once per strip.
         int tx0[4] = {0, 0, 0, 0}, tx1[4] = {0, 0, 0, 0};
         float tlx[4] = {0.f, 0.f, 0.f, 0.f};
         const float* dlo = depth;
         if (LOWRES) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) bilinear_taps(x + c, width, dw, tx0[c], tx1[c], tlx[c]);
+            for (int c = 0; c < 4; ++c)
+                bilinear_taps(x + c, width, dw, 1.0f / static_cast<float>(2 * width), tx0[c], tx1[c], tlx[c]);
             dlo = depth + static_cast<size_t>(f) * dh * dw;
         }
+        const float inv_2h = 1.0f / static_cast<float>(2 * height);
+        auto hrow = [&](int row) {
+            const float* p = dlo + static_cast<size_t>(row) * dw;
+            float v[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float a = __ldg(p + tx0[c]);
+                v[c] = fmaf(tlx[c], __ldg(p + tx1[c]) - a, a);
+            }
+            return make_float4(v[0], v[1], v[2], v[3]);
+        };
+        int it = -1, ib = -1, in = -1;                           // low-res rows held in top, bot, nxt
+        float4 top = make_float4(0.f, 0.f, 0.f, 0.f), bot = top, nxt = top;
         for (int y = ya; y < yb; y += U) {
             float4 d[U];
             if (HAS_DEPTH && !LOWRES) {
 #pragma unroll
                 for (int r = 0; r < U; ++r)
                     if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
-            }
-            if (LOWRES) {
-#pragma unroll
-                for (int r = 0; r < U; ++r) {
-                    if (y + r < yb) {
-                        int ty0, ty1;
-                        float ly;
-                        bilinear_taps(y + r, height, dh, ty0, ty1, ly);
-                        const float* r0 = dlo + static_cast<size_t>(ty0) * dw;
-                        const float* r1 = dlo + static_cast<size_t>(ty1) * dw;
-                        float v[4];
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) {
-                            const float top = fmaf(tlx[c], __ldg(r0 + tx1[c]) - __ldg(r0 + tx0[c]), __ldg(r0 + tx0[c]));
-                            const float bot = fmaf(tlx[c], __ldg(r1 + tx1[c]) - __ldg(r1 + tx0[c]), __ldg(r1 + tx0[c]));
-                            v[c] = fmaf(ly, bot - top, top);
-                        }
-                        d[r] = make_float4(v[0], v[1], v[2], v[3]);
-                    }
-                }
             }
 #pragma unroll
             for (int r = 0; r < U; ++r) {
@@ -734,6 +731,26 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
                             acc.z = fmaf(e[4 * q + k].z, wy[k], acc.z);
                             acc.w = fmaf(e[4 * q + k].w, wy[k], acc.w);
                         }
+                    }
+                    if (LOWRES) {
+                        int ty0, ty1;
+                        float ly;
+                        bilinear_taps(y + r, height, dh, inv_2h, ty0, ty1, ly);
+                        if (ty0 != it || ty1 != ib) {
+                            if (ty0 == ib && ty1 == in) {       // the usual step when upsampling: slide down one low-res row
+                                top = bot;
+                                bot = nxt;
+                            } else {
+                                top = hrow(ty0);
+                                bot = hrow(ty1);
+                            }
+                            it = ty0;
+                            ib = ty1;
+                            in = min(ib + 1, dh - 1);
+                            nxt = hrow(in);
+                        }
+                        d[r] = make_float4(fmaf(ly, bot.x - top.x, top.x), fmaf(ly, bot.y - top.y, top.y),
+                                           fmaf(ly, bot.z - top.z, top.z), fmaf(ly, bot.w - top.w, top.w));
                     }
                     const float4 m = make_float4(acc.x * scale, acc.y * scale, acc.z * scale, acc.w * scale);
                     const size_t o = img + static_cast<size_t>(y + r) * width;
@@ -894,6 +911,8 @@ extern "C" mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intr
         return mf::fail(MF_ERR_INVALID_ARG, "mf_motion_focus_upsampled: depth_lowres, focus_map and guided_depth are required");
     if (depth_width < 1 || depth_height < 1)
         return mf::fail(MF_ERR_INVALID_ARG, "mf_motion_focus_upsampled: bad depth size %dx%d", depth_width, depth_height);
+    if (width > 32767 || height > 32767 || depth_width > 32767 || depth_height > 32767)     // bilinear_taps works in int32
+        return mf::fail(MF_ERR_UNSUPPORTED, "mf_motion_focus_upsampled: sizes above 32767 are not supported");
     return motion_focus_impl(global_w2c, K, num_frames, render_begin, render_end, width, height, depth_lowres, depth_width,
                              depth_height, params, focus_map, guided_depth, focus_uv, focus_index, workspace, workspace_bytes, stream);
 }
