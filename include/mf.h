@@ -148,6 +148,26 @@ mf_status mf_motion_focus(const double* global_w2c, mf_intrinsics K, int num_fra
                           int32_t* focus_index, void* workspace, size_t workspace_bytes,
                           void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Depth alignment across windows and stitching of the emitted frames (Fig. 3 "Depth alignment"; emitted frames
+ * P:76).  The paper gives no formula for the depth scale (its pose alignment is rigid);
+ * reading F2 in DESIGN.md: window n >= 1 is brought to the scale of the stream so far by the least-squares factor on the
+ * frames it shares with window n-1,
+ *     r_n = sum D_{n-1} D_n / sum D_n^2   over pixels of the shared frames where both depths are finite and > 0
+ *           (r_n = 1 when there is none),      c_0 = 1,  c_n = c_{n-1} r_n,
+ * and frame t, emitted by window n at local index k, becomes depth_out[t] = fp32(c_n * depth_local[n][k]).
+ * depth_local: fp32 device [num_windows, W, height, width], each window in its own scale.  depth_out: fp32 device
+ * [num_frames, height, width].  window_scale: fp64 device [num_windows] receiving c_n, or NULL.  workspace:
+ * mf_align_depth_workspace_size(num_windows) bytes of device memory, 8-byte aligned.  Sums are fp64 in a fixed order:
+ * the result is deterministic.  Errors: num_windows != mf_num_windows(num_frames, W, stride), bad sizes, NULL or short
+ * workspace -> MF_ERR_INVALID_ARG.  Any height/width is accepted (16-byte vector path when height*width % 4 == 0 and the
+ * pointers are 16-byte aligned).
+ */
+size_t mf_align_depth_workspace_size(int num_windows);
+mf_status mf_align_depth(const float* depth_local, int num_windows, int W, int stride, int num_frames,
+                         int height, int width, float* depth_out, double* window_scale, void* workspace,
+                         size_t workspace_bytes, void* stream);
+
 /* mf_motion_focus with the depth at the MODEL's resolution (the paper does not say how its depth
  * maps reach the focus-map resolution, reading F1 in DESIGN.md): depth_lowres is fp32 [count, depth_height, depth_width]
  * and is interpolated inside the render pass, bilinear with half-pixel centres and edge clamping (what

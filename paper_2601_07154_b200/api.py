@@ -20,7 +20,8 @@ ACT_NONE, ACT_GELU = 0, 1
 EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", "mf_window_start",
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
            "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
-           "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step", "mf_motion_focus_upsampled"]
+           "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step", "mf_motion_focus_upsampled",
+           "mf_align_depth_workspace_size", "mf_align_depth"]
 
 
 class MfError(RuntimeError):
@@ -77,6 +78,9 @@ def lib():
         L.mf_chain_poses_step.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp]
         L.mf_motion_focus_upsampled.argtypes = [vp, Intrinsics, ci, ci, ci, ci, ci, vp, ci, ci, ctypes.POINTER(FocusParams),
                                                 vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
+        L.mf_align_depth_workspace_size.restype = ctypes.c_size_t
+        L.mf_align_depth_workspace_size.argtypes = [ci]
+        L.mf_align_depth.argtypes = [vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, ctypes.c_size_t, vp]
         _lib = L
     return _lib
 
@@ -140,6 +144,25 @@ def chain_poses(local_w2c, stride, num_frames, mode=ALIGN_YAW_TRANSLATION):
     out = torch.empty((seqs, num_frames, 4, 4), device=x.device, dtype=torch.float64)
     _check(lib().mf_chain_poses(_ptr(x), seqs, nw, w, stride, num_frames, mode, _ptr(out), _stream()))
     return out[0] if squeeze else out
+
+
+def align_depth(depth_local, stride, num_frames, workspace=None, out=None):
+    """depth_local: fp32 CUDA [num_windows, W, h, w], each window in its own scale -> (depth fp32 [N, h, w], c_n fp64 [Nw])."""
+    _dev(depth_local, torch.float32, "depth_local")
+    if depth_local.dim() != 4:
+        raise MfError("depth_local must be [num_windows, W, height, width]")
+    nw, w, h, wd = depth_local.shape
+    need = lib().mf_align_depth_workspace_size(nw)
+    if workspace is None:
+        workspace = torch.empty((need,), device=depth_local.device, dtype=torch.uint8)
+    if out is None:
+        out = torch.empty((num_frames, h, wd), device=depth_local.device, dtype=torch.float32)
+    else:
+        _dev(out, torch.float32, "out")
+    scales = torch.empty((nw,), device=depth_local.device, dtype=torch.float64)
+    _check(lib().mf_align_depth(_ptr(depth_local), nw, w, stride, num_frames, h, wd, _ptr(out), _ptr(scales), _ptr(workspace),
+                                workspace.numel(), _stream()))
+    return out, scales
 
 
 def focus_params(n_points=15, sigma=20.0, vec=VEC_ACCEL, mag=MAG_UNIT, norm=NORM_MAX, pts=PTS_CURRENT_FRAME,

@@ -138,6 +138,25 @@ def depth(frames, height, width, seed, device="cpu"):
                       dtype=torch.float32) * 29.0 + 1.0
 
 
+def depth_windows(num_frames, w, stride, height, width, seed, gauge_spread=2.0, noise=0.02, invalid=0.0):
+    """Window-local depth maps, fp32 numpy [Nw, W, height, width]: one Uniform(1, 30) m stream, cut into windows, each window
+    divided by its own scale (log-uniform in [1/gauge_spread, gauge_spread]) and multiplied by per-pixel noise
+    (1 + noise * N(0,1)), so that overlapping estimates disagree like a model's would.  A fraction `invalid` of the pixels is
+    replaced by 0, NaN or inf (sky / holes).  Returns (depth_local, gauges)."""
+    rng = np.random.default_rng(seed)
+    stream = rng.uniform(1.0, 30.0, (num_frames, height, width))
+    starts = window_starts(num_frames, w, stride)
+    gauges = np.exp(rng.uniform(-np.log(gauge_spread), np.log(gauge_spread), len(starts)))
+    out = np.empty((len(starts), w, height, width), dtype=np.float32)
+    for i, s0 in enumerate(starts):
+        d = stream[s0:s0 + w] / gauges[i] * (1.0 + noise * rng.standard_normal((w, height, width)))
+        if invalid > 0.0:
+            bad = rng.uniform(size=d.shape) < invalid
+            d[bad] = rng.choice(np.array([0.0, np.nan, np.inf, -1.0]), size=int(bad.sum()))
+        out[i] = d.astype(np.float32)
+    return out, gauges
+
+
 def tokens(m, d, seed, device="cpu"):
     """Activations ~ N(0,1) rounded to bf16, [m, d]."""
     import torch

@@ -1,0 +1,96 @@
+"""GPU parity: mf_align_depth (through the C ABI) vs oracle/depth.py (reading F2).
+Bars: window scales c_n within 1e-12 relative (both sides sum exact fp64 products, in different orders); stitched depth within
+1e-6 relative (one fp32 rounding of c_n * D, plus the c_n difference); invalid pixels propagate as the product defines."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import depth as od
+from oracle import render as orr
+from oracle import windows as ow
+from paper_2601_07154_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2601_07154_b200 import api as a
+    a.lib()
+    return a
+
+
+def _case(api, n, w, stride, h, wd, seed, **kw):
+    loc, _ = synth.depth_windows(n, w, stride, h, wd, seed, **kw)
+    ref, c_ref = od.align_depth(loc, w, stride, n)
+    got, c = api.align_depth(torch.from_numpy(loc).cuda(), stride, n)
+    torch.cuda.synchronize()
+    got, c = got.cpu().numpy(), c.cpu().numpy()
+    assert np.abs(c - c_ref).max() <= 1e-12 * np.abs(c_ref).max(), (c, c_ref)
+    fin = np.isfinite(ref)
+    assert np.array_equal(np.isnan(got), np.isnan(ref)) and np.array_equal(np.isinf(got), np.isinf(ref))
+    assert np.abs(got[fin] - ref[fin]).max() <= 1e-6 * np.abs(ref[fin]).max()
+    assert (np.abs(got[fin] - ref[fin]) <= 1e-6 * np.abs(ref[fin]) + 1e-30).all()
+    return loc, got, c
+
+
+@pytest.mark.parametrize("n,w,stride,h,wd", [
+    (4, 4, 2, 8, 8),            # one window: pass-through
+    (12, 4, 2, 6, 10),          # regular strides, vector path
+    (13, 4, 2, 7, 9),           # tail window (larger last overlap), scalar path (63 pixels)
+    (23, 8, 7, 5, 12),          # overlap of one frame
+    (9, 5, 1, 4, 4),            # stride 1
+    (48, 32, 16, 294, 518),     # the BJ campus window at the model's resolution: many tiles, ragged vector tail
+    (100, 16, 8, 37, 41),       # odd sizes
+])
+def test_align_depth_parity(api, n, w, stride, h, wd):
+    _case(api, n, w, stride, h, wd, seed=11 + n)
+
+
+def test_align_depth_recovers_gauges_and_ignores_invalid_pixels(api):
+    n, w, stride = 40, 8, 4
+    loc, g = synth.depth_windows(n, w, stride, 16, 20, 5, noise=0.0)
+    got, c = api.align_depth(torch.from_numpy(loc).cuda(), stride, n)
+    assert np.abs(c.cpu().numpy() - g / g[0]).max() <= 1e-6        # fp32 inputs: the gauges come back to fp32 accuracy
+    _case(api, n, w, stride, 16, 20, 6, invalid=0.2)               # zeros, NaN, inf, negatives in both windows
+    # nothing valid on an overlap: that window keeps the scale of the previous one
+    loc2 = loc.copy()
+    off = ow.window_starts(n, w, stride)
+    loc2[3, :w - stride] = np.nan
+    ref, c_ref = od.align_depth(loc2, w, stride, n)
+    _, c2 = api.align_depth(torch.from_numpy(loc2).cuda(), stride, n)
+    c2 = c2.cpu().numpy()
+    assert c2[3] == c2[2] and np.abs(c2 - c_ref).max() <= 1e-12 * np.abs(c_ref).max() and len(off) == len(c2)
+
+
+def test_align_depth_is_deterministic_and_feeds_the_focus_call(api):
+    n, w, stride, h, wd = 48, 32, 16, 294, 518
+    loc, _ = synth.depth_windows(n, w, stride, h, wd, 3)
+    x = torch.from_numpy(loc).cuda()
+    a, ca = api.align_depth(x, stride, n)
+    b, cb = api.align_depth(x, stride, n)
+    assert torch.equal(a, b) and torch.equal(ca, cb)
+    # stitched model-resolution depth -> mf_motion_focus_upsampled: the guided depth is the focus map times the upsampled stream
+    cfg = synth.CONFIGS[3]
+    poses = torch.from_numpy(np.asarray(synth.trajectory(cfg, 1, n))).cuda()
+    out = api.motion_focus_upsampled(poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"],
+                                     a[40:42].contiguous(),
+                                     api.focus_params(n_points=15, sigma=cfg["sigma"]), render_begin=40, render_end=42)
+    torch.cuda.synchronize()
+    assert out["focus_map"].max() > 0
+    for f in range(2):
+        up = orr.upsample_bilinear(a[40 + f].cpu().numpy(), cfg["width"], cfg["height"])      # fp64, reading F1
+        want = out["focus_map"][f].cpu().numpy().astype(np.float64) * up
+        assert np.abs(out["guided_depth"][f].cpu().numpy() - want).max() <= 1e-5 * np.abs(want).max()
+
+
+def test_align_depth_argument_errors(api):
+    x = torch.ones((3, 4, 2, 2), device="cuda")
+    with pytest.raises(api.MfError):
+        api.align_depth(x, 2, 9)                       # 9 frames with W=4, stride=2 make 4 windows, not 3
+    with pytest.raises(api.MfError):
+        api.align_depth(x, 4, 8)                       # stride >= W
+    with pytest.raises(api.MfError):
+        api.align_depth(x.double(), 2, 8)
+    with pytest.raises(api.MfError):
+        api.align_depth(x, 2, 8, workspace=torch.empty((8,), device="cuda", dtype=torch.uint8))
