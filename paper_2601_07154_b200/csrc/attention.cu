@@ -22,6 +22,7 @@
 #include "common.h"
 #include "sm100_ptx.cuh"
 #include "tensormap.h"
+#include "attention_common.cuh"
 
 #include <cuda_bf16.h>
 
@@ -58,16 +59,6 @@ struct AttnSmem {
     uint32_t zero;     // always 0 (see the softmax loop)
 };
 
-struct AttnParams {
-    int seq_len;        // tokens per attention sequence (S, or P in frame mode)
-    int heads;
-    int q_blocks;       // ceil(seq_len / 256)
-    float scale_log2;   // softmax_scale * log2(e)
-    __nv_bfloat16* out;
-    float* lse;         // [windows, heads, S] or nullptr
-    int lse_frames;     // sequences per window (W in frame mode, 1 in global mode)
-};
-
 constexpr uint32_t kIdescQK = ptx::idesc_bf16_f32(kBM, kBN, 0, 0);
 constexpr uint32_t kIdescPV = ptx::idesc_bf16_f32(kBM, kON, 0, 1);      // V is MN-major ([keys][d], d contiguous)
 
@@ -87,30 +78,6 @@ __device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, 
 #pragma unroll
     for (int i = 0; i < kBN / 32; ++i)
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
-}
-
-// (2^x0, 2^x1) on the FMA pipe.  x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a cubic (minimax in
-// relative error, 7.5e-5); n is added into the exponent field.  x is clamped to >= -125 so the result stays normal.
-__device__ __forceinline__ void exp2_poly2(uint32_t& a0, uint32_t& a1) {
-    const float x0 = fmaxf(__uint_as_float(a0), -125.0f), x1 = fmaxf(__uint_as_float(a1), -125.0f);
-    const uint64_t magic = ptx::pack2(12582912.0f, 12582912.0f);          // 1.5 * 2^23: x + magic holds round(x) in its low bits
-    const uint64_t c3 = ptx::pack2(0.055171407759189606f, 0.055171407759189606f);
-    const uint64_t c2 = ptx::pack2(0.24261075258255005f, 0.24261075258255005f);
-    const uint64_t c1 = ptx::pack2(0.6932609677314758f, 0.6932609677314758f);
-    const uint64_t c0 = ptx::pack2(0.9999281167984009f, 0.9999281167984009f);
-    const uint64_t x = ptx::pack2(x0, x1);
-    uint64_t t, n, f, p;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(x), "l"(magic));
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(n) : "l"(t), "l"(magic));
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(f) : "l"(x), "l"(n));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(c3), "l"(f), "l"(c2));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c1));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c0));
-    uint32_t p0, p1, t0, t1;
-    asm("mov.b64 {%0, %1}, %2;" : "=r"(p0), "=r"(p1) : "l"(p));
-    asm("mov.b64 {%0, %1}, %2;" : "=r"(t0), "=r"(t1) : "l"(t));
-    a0 = p0 + (t0 << 23);
-    a1 = p1 + (t1 << 23);
 }
 
 __device__ __forceinline__ void fadd2_acc(uint64_t& acc, uint32_t a0, uint32_t a1) {
@@ -404,7 +371,8 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
         return fail(MF_ERR_INVALID_ARG, "mf_window_attention: non-positive dimension");
     if (mode != MF_ATTN_GLOBAL && mode != MF_ATTN_FRAME)
         return fail(MF_ERR_INVALID_ARG, "mf_window_attention: bad mode %d", static_cast<int>(mode));
-    if (head_dim != kD) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: head_dim=%d (only 64 is built)", head_dim);
+    if (head_dim != kD && head_dim != 128)
+        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: head_dim=%d (64 and 128 are built)", head_dim);
     if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out))
         return fail(MF_ERR_ALIGNMENT, "mf_window_attention: q/k/v/out must be 16-byte aligned");
     if (out == q || out == k || out == v) return fail(MF_ERR_INVALID_ARG, "mf_window_attention: out aliases an input");
@@ -419,11 +387,6 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
         return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: sequence length / count too large");
     const int sequences = static_cast<int>(sequences_ll), seq_len = static_cast<int>(seq_len_ll);
 
-    CUtensorMap mq, mk, mv;
-    if ((st = make_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
-    if ((st = make_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
-    if ((st = make_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
-
     AttnParams prm;
     prm.seq_len = seq_len;
     prm.heads = heads;
@@ -433,6 +396,13 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     prm.out = static_cast<__nv_bfloat16*>(out);
     prm.lse = lse;
     prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
+    if (head_dim == 128)       // re-tiled variant (attention_d128.cu); q_blocks is the same: 256 query rows per CTA
+        return launch_attention_d128(q, k, v, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
+
+    CUtensorMap mq, mk, mv;
+    if ((st = make_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = make_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = make_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
     if (grid > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;

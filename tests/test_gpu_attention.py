@@ -23,8 +23,8 @@ def _to64(t):
     return t.detach().float().cpu().numpy().astype(np.float64)
 
 
-def _check(api, windows, w, p, heads, mode, seed, scale=1.0, rows=None, softmax_scale=0.0, lse=False):
-    q, k, v = synth.qkv(windows, w * p, heads, 64, seed, device="cuda", scale=1.0)
+def _check(api, windows, w, p, heads, mode, seed, scale=1.0, rows=None, softmax_scale=0.0, lse=False, dim=64):
+    q, k, v = synth.qkv(windows, w * p, heads, dim, seed, device="cuda", scale=1.0)
     if scale != 1.0:
         q = (q.float() * scale).to(torch.bfloat16)
     res = api.window_attention(q, k, v, w, p, mode, softmax_scale, return_lse=lse)
@@ -163,6 +163,46 @@ def _random_cases(n, seed):
 def test_random_shapes(api, windows, w, p, heads, mode, qscale, seed):
     # seeded random (windows, W, P, heads, mode, score scale): tiles, ragged tails and frame boundaries land anywhere
     _check(api, windows, w, p, heads, mode, seed, scale=qscale, lse=True)
+
+
+# ---- head_dim 128: 64-key KV tiles, two swizzle atoms per row, 3-stage ring ----
+@pytest.mark.parametrize("windows,w,p,heads", [
+    (2, 3, 100, 2),      # S=300: two Q tiles, second ragged; ragged last KV tile
+    (1, 1, 64, 1),       # exactly one KV tile
+    (1, 1, 65, 1),       # one key into the second KV tile
+    (1, 1, 129, 1),      # one row into the second Q tile
+    (3, 2, 64, 3),
+    (1, 5, 77, 2),       # S=385: 2 CTAs per head, ragged everywhere
+    (1, 1, 1, 1),
+    (1, 7, 64, 1),       # S=448 = 7 KV tiles: ring wraps (3 stages) with phase flips
+    (1, 4, 256, 8),      # the tiny config's sequence at head_dim 128
+])
+@pytest.mark.parametrize("mode", [oa.GLOBAL, oa.FRAME])
+def test_head_dim_128_shapes(api, windows, w, p, heads, mode):
+    _check(api, windows, w, p, heads, mode, 4321 + windows * 7 + w * 13 + p, lse=True, dim=128)
+
+
+@pytest.mark.parametrize("qscale", [2.0, 4.0])
+def test_head_dim_128_peaked_and_rescale(api, qscale):
+    _check(api, 1, 4, 256, 4, oa.GLOBAL, 987, scale=qscale, lse=True, dim=128)
+    # running maximum grows tile after tile: forces the O / l rescale through TMEM (4 x 32 columns + the sum column)
+    s_len = 1024
+    q = (torch.ones((1, s_len, 1, 128), device="cuda") * 0.35).to(torch.bfloat16)
+    ramp = torch.linspace(-6, 6, s_len, device="cuda")[None, :, None, None]
+    k = (ramp * torch.ones((1, s_len, 1, 128), device="cuda")).to(torch.bfloat16)
+    g = torch.Generator(device="cuda").manual_seed(6)
+    v = torch.randn((1, s_len, 1, 128), device="cuda", generator=g).to(torch.bfloat16)
+    out = api.window_attention(q, k, v, 4, 256)
+    ref, _ = oa.window_attention(_to64(q), _to64(k), _to64(v), 4, 256)
+    d = _to64(out) - ref
+    assert np.abs(d).max() <= MAX_ABS and np.linalg.norm(d) / np.linalg.norm(ref) <= REL_L2
+
+
+def test_head_dim_128_long_sequence_sampled_rows(api):
+    # S = 6216 (the suburban window) at head_dim 128, oracle on a sampled row set (reading A7)
+    w, p = 8, 777
+    rows = _a7_rows(w, p, 31)
+    _check(api, 1, w, p, 2, oa.GLOBAL, 55, rows=rows, lse=True, dim=128)
 
 
 def test_errors(api):
