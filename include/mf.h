@@ -26,7 +26,7 @@ extern "C" {
 typedef enum {
     MF_OK = 0,
     MF_ERR_INVALID_ARG = 1,   /* bad dimension / enum / NULL pointer                    */
-    MF_ERR_UNSUPPORTED = 2,   /* valid request this build cannot run (head_dim != 64...) */
+    MF_ERR_UNSUPPORTED = 2,   /* valid request this build cannot run (head_dim not 64 or 128...) */
     MF_ERR_ALIGNMENT = 3,     /* pointer not 16-byte aligned, width % 4 != 0            */
     MF_ERR_WORKSPACE = 4,     /* workspace NULL or too small                             */
     MF_ERR_CUDA = 5           /* CUDA runtime / driver error, no sm_100 device           */
@@ -49,7 +49,7 @@ int mf_version(void);         /* major*10000 + minor*100 + patch */
  * q,k,v,out: bf16 [windows, S, heads, head_dim] contiguous, 16-byte aligned; out must not
  * alias q/k/v.  lse: optional fp32 [windows, heads, S] natural-log-sum-exp of the scaled
  * scores (accurate to 2^-8 absolute: it is formed from the bf16-rounded weights the PV product
- * uses), or NULL.  head_dim must be 64 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
+ * uses), or NULL.  head_dim must be 64 or 128 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
  * selects 1/sqrt(head_dim).
  */
 typedef enum { MF_ATTN_GLOBAL = 0, MF_ATTN_FRAME = 1 } mf_attn_mode;
