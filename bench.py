@@ -34,6 +34,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stream", action="store_true", help="skip the per-window streaming latency measurement (SURVEY 8(f) NEXT-2)")
+    ap.add_argument("--no-d128", action="store_true", help="skip the head_dim 128 attention measurement (SURVEY 8(f) NEXT-3)")
     ap.add_argument("--no-block", action="store_true", help="skip the whole-transformer-block measurement (SURVEY 8(f) NEXT-1)")
     return ap.parse_args()
 
@@ -270,6 +271,31 @@ def measure_block(wl, torch, api):
     pair_ms = out["frame_block_ms"] + out["global_block_ms"]
     out["frames_per_s_full_blocks"] = wl.N / (pair_ms * 1e-3 * (wl.layers // 2) * ((wl.Nw + wl.B - 1) // wl.B))
     return out
+
+
+def measure_d128(wl, torch, api, peak_sustained):
+    """SURVEY 8(f) NEXT-3 (not part of the headline step): the GLOBAL attention launch of this workload at head_dim 128 with
+    half the heads (same d_model, same S, same windows per launch), 0.5 s of back-to-back launches after warm-up."""
+    from paper_2601_07154_b200 import synth
+    heads = max(1, wl.H * wl.D // 128)
+    q, k, v = synth.qkv(wl.B, wl.S, heads, 128, synth.seed_for(wl.cfg_idx, 8), device=wl.device)
+    o = torch.empty_like(q)
+    flops = 4.0 * wl.S * wl.S * heads * 128 * wl.B
+    for _ in range(3):
+        api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+    torch.cuda.synchronize()
+    n = 50 if wl.S >= 8192 else 200
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n):
+        api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / n
+    tf = flops / (ms * 1e-3) / 1e12
+    return {"what": "mf_window_attention GLOBAL at head_dim 128 (SURVEY 8(f) NEXT-3; not in the headline step)", "heads": heads,
+            "seq_len": wl.S, "windows_per_launch": wl.B, "launches": n, "ms_per_launch": ms, "tflops": tf,
+            "frac_of_sustained_peak": tf / peak_sustained}
 
 
 def measure_streaming(wl, torch, api):
@@ -511,6 +537,10 @@ def main():
     if rank == 0 and not args.no_block and wl.layers > 1:
         block = measure_block(wl, torch, api)
 
+    d128 = None
+    if rank == 0 and not args.no_d128 and wl.D == 64:
+        d128 = measure_d128(wl, torch, api, peaks["tf_sustained"])
+
     streaming = None
     if rank == 0 and not args.no_stream and wl.Nw >= 8 and wl.layers > 1:
         streaming = measure_streaming(wl, torch, api)
@@ -522,7 +552,7 @@ def main():
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
                 "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
-                "cpu_baseline": cpu, "e2e": e2e, "block": block, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+                "cpu_baseline": cpu, "e2e": e2e, "block": block, "head_dim_128": d128, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
         print(json.dumps(line))
     replicas.finish()
 

@@ -9,7 +9,7 @@
 // every tile is stored as a low and a high 64-column half (two TMA boxes).  QK^T runs 8 K=16 steps, 4 in each half.  For
 // O += P [V_lo | V_hi | ones] (M=128, N=144, MN-major B) the three 64-column atoms of a stage lie 8 KB apart (LBO), which is why
 // every V stage carries its own copy of the ones tile.
-// Per 64 keys and CTA the tensor pipe has 1088 clk of work (QK 512, PV 576) against 768-1024 clk on the exponent unit:
+// Per 64 keys and CTA the tensor pipe has 1088 clk of work (QK 512, PV 576) against 1024 clk on the exponent unit:
 // at head_dim 128 the tensor core, not MUFU, is the first pipe to saturate.
 #include "attention_common.cuh"
 #include "tensormap.h"
@@ -34,7 +34,7 @@ constexpr int kON = kD + 16;           // PV accumulator columns: 128 outputs + 
 constexpr int kPCols = kBN / 2;        // TMEM columns of one P tile (64 keys, bf16)
 constexpr float kRescaleThreshold = 8.0f;
 #ifndef MF_POLY_PAIRS_D128
-#define MF_POLY_PAIRS_D128 4           // of every 16 score pairs, this many are exponentiated on the FMA pipe
+#define MF_POLY_PAIRS_D128 0           // of every 16 score pairs, this many are exponentiated on the FMA pipe (measured: 0 is best here)
 #endif
 constexpr int kPolyPairs = MF_POLY_PAIRS_D128;
 
