@@ -327,8 +327,10 @@ static mf_status make_map(CUtensorMap* map, const void* base, int sequences, int
 }  // namespace d128
 
 mf_status launch_attention_d128(const void* q, const void* k, const void* v, int sequences, int seq_len, int heads,
-                                const AttnParams& prm, cudaStream_t stream) {
+                                const AttnParams& prm_in, cudaStream_t stream) {
     using namespace d128;
+    AttnParams prm = prm_in;
+    prm.q_blocks = (seq_len + kQTiles * kBM - 1) / (kQTiles * kBM);
     CUtensorMap mq, mk, mv;
     mf_status st;
     if ((st = make_map(&mq, q, sequences, seq_len, heads, kBM)) != MF_OK) return st;
