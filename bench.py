@@ -322,9 +322,13 @@ def measure_streaming(wl, torch, api):
     def load(n):
         q.copy_(wl.q[n:n + 1]); k.copy_(wl.k[n:n + 1]); v.copy_(wl.v[n:n + 1]); win.copy_(wl.local[n])
 
-    def step(first=False):
+    def attention():
         for layer in range(wl.layers):
             api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_FRAME if layer % 2 == 0 else api.ATTN_GLOBAL, out=o[layer % 2])
+
+    def step(first=False, with_attention=True):
+        if with_attention:
+            attention()
         if first:
             full = api.chain_poses_step(win, state, first=True)
             ring[-wl.W:].copy_(full)
@@ -361,9 +365,54 @@ def measure_streaming(wl, torch, api):
     torch.cuda.current_stream().wait_stream(side)
     torch.cuda.synchronize()
     graph_ms = timed(graph.replay, range(5, 8))
+
+    # Overlapped form: the attention stack of window n+1 runs on the main stream while the chain step and the focus render of
+    # window n run on a second stream (two graphs; q,k,v are only touched on the main stream, the window-local poses only on
+    # the second one).  Steady-state time per window over 6 windows back to back, against the single graph timed the same way.
+    main = torch.cuda.current_stream()
+    tail_stream = torch.cuda.Stream(device=dev)
+    g_attn, g_tail = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+    side.wait_stream(main)
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g_attn, stream=side):
+            attention()
+        with torch.cuda.graph(g_tail, stream=side):
+            step(with_attention=False)
+    main.wait_stream(side)
+    torch.cuda.synchronize()
+
+    def run_serial(n):
+        load(n)
+        graph.replay()
+
+    def run_overlapped(n):
+        q.copy_(wl.q[n:n + 1]); k.copy_(wl.k[n:n + 1]); v.copy_(wl.v[n:n + 1])
+        g_attn.replay()
+        done = torch.cuda.Event()
+        done.record(main)
+        with torch.cuda.stream(tail_stream):
+            tail_stream.wait_event(done)
+            win.copy_(wl.local[n])
+            g_tail.replay()
+
+    def back_to_back(fn, windows):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(main)
+        for n in windows:
+            fn(n)
+        main.wait_stream(tail_stream)
+        e1.record(main)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / len(windows)
+
+    nwin = list(range(2, min(wl.Nw, 8)))
+    back_to_back(run_overlapped, nwin[:2])
+    serial_ms = back_to_back(run_serial, nwin)
+    overlap_ms = back_to_back(run_overlapped, nwin)
     return {"what": f"one window at a time (SURVEY 8(f) NEXT-2; not in the headline step): {wl.layers} attention launches + "
                     "mf_chain_poses_step + rolling pose buffer + mf_motion_focus of the new frames",
             "new_frames_per_window": m, "eager_ms_per_window": eager_ms, "graph_ms_per_window": graph_ms,
+            "graph_back_to_back_ms_per_window": serial_ms, "two_stream_overlap_ms_per_window": overlap_ms,
             "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
 
 

@@ -80,12 +80,6 @@ __device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, 
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
 }
 
-__device__ __forceinline__ void fadd2_acc(uint64_t& acc, uint32_t a0, uint32_t a1) {
-    uint64_t x;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "r"(a0), "r"(a1));
-    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(x));
-}
-
 __global__ void __launch_bounds__(kThreads, 1)
 window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                         const __grid_constant__ CUtensorMap map_v, const AttnParams prm) {
