@@ -14,6 +14,7 @@ sys.path.insert(0, ROOT)
 from oracle import attention as oa          # noqa: E402
 from oracle import block as ob              # noqa: E402
 from oracle import chain as oc              # noqa: E402
+from oracle import depth as od              # noqa: E402
 from oracle import points as op             # noqa: E402
 from oracle import render as orr            # noqa: E402
 
@@ -44,6 +45,11 @@ def build():
     loc = np.stack([np.array(poses[0:4]), np.array(poses[2:6]), np.array(poses[4:8])]).astype(np.float32)
     chained = np.array(oc.chain_poses(loc.tolist(), 4, 2, 8))
     x = rng.standard_normal((3, 8))
+    up = orr.upsample_bilinear(rng.uniform(1.0, 9.0, (3, 4)), 10, 7)
+    dloc = rng.uniform(1.0, 9.0, (3, 4, 2, 3))
+    dloc[1] *= 0.5
+    dloc[2] *= 3.0
+    d_out, d_scales = od.align_depth(dloc, 4, 2, 8)
     return {
         "attention_global_o": np.round(o_g, 12).tolist(), "attention_global_lse": np.round(lse_g, 12).tolist(),
         "attention_frame_o_row0": np.round(o_f[0, 0], 12).tolist(),
@@ -53,6 +59,8 @@ def build():
         "gelu": np.round(ob.gelu(x[0]), 12).tolist(),
         "layernorm_row0": np.round(ob.layernorm(x, np.ones(8), np.zeros(8))[0], 12).tolist(),
         "round_bf16": ob.round_bf16(x[1]).tolist(),
+        "upsample_bilinear_row3": np.round(up[3], 12).tolist(),
+        "align_depth_scales": np.round(d_scales, 12).tolist(), "align_depth_last_frame": np.round(d_out[-1], 12).tolist(),
     }
 
 
