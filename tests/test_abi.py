@@ -63,6 +63,15 @@ def test_argument_errors_need_no_device(lib):
     assert lib.mf_chain_poses(p, 1, 1, 4, 4, 4, 0, q, None) == 1                               # stride >= W
     assert lib.mf_motion_focus_workspace_size(1, 224, 224, 33) == 0
     assert lib.mf_motion_focus_workspace_size(2, 224, 224, 15) > 2 * 16 * 448 * 4
+    # mf_align_depth / mf_motion_focus_upsampled: every check below is made before the device is touched
+    assert lib.mf_align_depth_workspace_size(0) == 0 and lib.mf_align_depth_workspace_size(3) >= 3 * 8
+    ws = lib.mf_align_depth_workspace_size(3)
+    assert lib.mf_align_depth(None, 3, 4, 2, 8, 2, 2, q, None, p, ws, None) == 1 and b"NULL" in lib.mf_last_error()
+    assert lib.mf_align_depth(p, 2, 4, 2, 8, 2, 2, q, None, p, ws, None) == 1                  # 8 frames, W=4, stride 2: 3 windows
+    assert lib.mf_align_depth(p, 3, 4, 4, 8, 2, 2, q, None, p, ws, None) == 1                  # stride >= W
+    assert lib.mf_align_depth(p, 3, 4, 2, 8, 0, 2, q, None, p, ws, None) == 1                  # empty image
+    assert lib.mf_align_depth(p, 3, 4, 2, 8, 2, 2, q, None, p, 8, None) == 1                   # workspace too small
+    assert lib.mf_align_depth(p, 3, 4, 2, 8, 2, 2, q, None, None, ws, None) == 1
 
 
 def test_missing_library_fails_loudly(monkeypatch):
