@@ -240,7 +240,7 @@ mf_status mf_layernorm(const void* x, const float* gamma, const float* beta, flo
  *   w_qkv [3 d, d] (rows: q | k | v, each head-major), w_o [d, d], w_1 [d_hidden, d], w_2 [d, d_hidden].
  * Every tensor kept between two kernels is bf16 (E5).  Seven launches: layernorm, linear (q|k|v), window attention,
  * linear (+residual), layernorm, linear (+GELU), linear (+residual).  d = heads * head_dim must be 256, 512, 768 or
- * 1024 with head_dim 64, d_hidden % 256 == 0.  workspace: mf_block_workspace_size() bytes of device memory.
+ * 1024 with head_dim 64 or 128, d_hidden % 256 == 0.  workspace: mf_block_workspace_size() bytes of device memory.
  */
 typedef struct {
     const float* ln1_gamma; const float* ln1_beta;

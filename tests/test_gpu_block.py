@@ -98,14 +98,14 @@ def test_linear_errors(api):
 
 
 @pytest.mark.parametrize("mode_name", ["global", "frame"])
-@pytest.mark.parametrize("windows,w,p,heads,d_hidden", [(2, 2, 100, 4, 1024), (1, 3, 77, 8, 768)])
-def test_block_forward_vs_oracle(api, windows, w, p, heads, d_hidden, mode_name):
+@pytest.mark.parametrize("windows,w,p,heads,d_hidden,head_dim", [(2, 2, 100, 4, 1024, 64), (1, 3, 77, 8, 768, 64), (1, 2, 150, 4, 1024, 128)])
+def test_block_forward_vs_oracle(api, windows, w, p, heads, d_hidden, head_dim, mode_name):
     # whole pre-norm block (E1, E2) with bf16 storage between kernels (E5): 7 launches vs oracle.block.block_forward.
     # Intermediate bf16 tensors may differ from the oracle's by rare 1-ulp rounding flips (fp32 vs fp64 sums landing on
     # either side of a rounding boundary); a flipped h plus y's own rounding is 2 bf16 ulps = 2^-6 |ref| on a few elements.
     from oracle import attention as oa
     mode = oa.GLOBAL if mode_name == "global" else oa.FRAME
-    d = heads * 64
+    d = heads * head_dim
     s_len = w * p
     x = synth.tokens(windows * s_len, d, seed=7 + windows + heads, device="cuda")
     wts = synth.block_weights(d, d_hidden, seed=11 + heads, device="cuda")
