@@ -205,6 +205,20 @@ def test_head_dim_128_long_sequence_sampled_rows(api):
     _check(api, 1, w, p, 2, oa.GLOBAL, 55, rows=rows, lse=True, dim=128)
 
 
+@pytest.mark.parametrize("windows,w,p,heads,mode,qscale,seed", _random_cases(16, 20260108))
+def test_head_dim_128_random_shapes(api, windows, w, p, heads, mode, qscale, seed):
+    _check(api, windows, w, p, heads, mode, seed, scale=min(qscale, 2.0), lse=True, dim=128)
+
+
+def test_head_dim_128_determinism_at_scale(api):
+    # races show up as run-to-run differences: 2 campus windows, 8 heads of 128, both modes
+    q, k, v = synth.qkv(2, 32 * 777, 8, 128, 5, device="cuda")
+    for mode in (oa.GLOBAL, oa.FRAME):
+        ref = api.window_attention(q, k, v, 32, 777, mode)
+        for _ in range(4):
+            assert torch.equal(api.window_attention(q, k, v, 32, 777, mode), ref)
+
+
 def test_errors(api):
     q, k, v = synth.qkv(1, 64, 1, 32, 1, device="cuda")
     with pytest.raises(api.MfError):

@@ -84,6 +84,21 @@ def test_align_depth_is_deterministic_and_feeds_the_focus_call(api):
         assert np.abs(out["guided_depth"][f].cpu().numpy() - want).max() <= 1e-5 * np.abs(want).max()
 
 
+def _random_depth_cases(count, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(count):
+        w = int(rng.integers(2, 12))
+        out.append((w + int(rng.integers(0, 40)), w, int(rng.integers(1, w)), int(rng.integers(1, 40)), int(rng.integers(1, 60)),
+                    float(rng.choice([0.0, 0.1])), int(rng.integers(1 << 30))))
+    return out
+
+
+@pytest.mark.parametrize("n,w,stride,h,wd,invalid,seed", _random_depth_cases(12, 20260109))
+def test_align_depth_random_shapes(api, n, w, stride, h, wd, invalid, seed):
+    _case(api, n, w, stride, h, wd, seed, invalid=invalid)
+
+
 def test_align_depth_argument_errors(api):
     x = torch.ones((3, 4, 2, 2), device="cuda")
     with pytest.raises(api.MfError):
