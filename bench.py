@@ -416,7 +416,7 @@ def measure_streaming(wl, torch, api):
             "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
 
 
-def oracle_sample(cfg_idx, wl_dims, rows=1024):
+def oracle_sample(cfg_idx, wl_dims, rows=4096):
     """Times the oracle, as it stands, on a bounded sample of the same workload (host cores) and
     extrapolates to the whole clip.  Returns (frames_per_s, seconds_of_sample, description, cores)."""
     import numpy as np
