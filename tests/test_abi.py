@@ -72,6 +72,14 @@ def test_argument_errors_need_no_device(lib):
     assert lib.mf_align_depth(p, 3, 4, 2, 8, 0, 2, q, None, p, ws, None) == 1                  # empty image
     assert lib.mf_align_depth(p, 3, 4, 2, 8, 2, 2, q, None, p, 8, None) == 1                   # workspace too small
     assert lib.mf_align_depth(p, 3, 4, 2, 8, 2, 2, q, None, None, ws, None) == 1
+    from paper_2601_07154_b200 import api
+    k = api.Intrinsics(100.0, 100.0, 16.0, 12.0)
+    prm = api.focus_params()
+    up = lambda **kw: lib.mf_motion_focus_upsampled(p, k, 4, 0, 4, kw.get("w", 32), kw.get("h", 24), kw.get("d", p), kw.get("dw", 8),
+                                                    kw.get("dh", 6), ctypes.byref(prm), q, kw.get("g", q), None, None, p, 1 << 20, None)
+    assert up(d=None) == 1 and up(g=None) == 1                 # depth_lowres and guided_depth are required
+    assert up(dw=0) == 1 and up(dh=-3) == 1                     # bad depth size
+    assert up(dw=40000) == 2 and up(w=40000) == 2               # sizes above 32767: MF_ERR_UNSUPPORTED
 
 
 def test_missing_library_fails_loudly(monkeypatch):
