@@ -168,6 +168,19 @@ mf_status mf_align_depth(const float* depth_local, int num_windows, int W, int s
                          int height, int width, float* depth_out, double* window_scale, void* workspace,
                          size_t workspace_bytes, void* stream);
 
+/* Streaming form of mf_align_depth (one window per call, as mf_chain_poses_step).  state:
+ * mf_align_depth_state_size() bytes of device memory, 8-byte aligned, contents irrelevant before the first window; it holds
+ * c_{n-1} and is updated in place.  first_window != 0: c_0 = 1 and all W frames of cur_window are emitted.  Otherwise
+ * prev_window is the previous window's [W, height, width] depth (unscaled, as the model produced it), the two windows share
+ * the last W - new_frames frames of prev_window = the first W - new_frames frames of cur_window (1 <= new_frames < W), and the
+ * last new_frames frames of cur_window are emitted, scaled by c_n.  depth_out: fp32 device [emitted, height, width].  Same sums
+ * in the same order as mf_align_depth: feeding the windows of a clip one by one reproduces its output bit for bit (given the
+ * same 16-byte alignment of the window buffers, which selects the vector path).
+ */
+size_t mf_align_depth_state_size(void);
+mf_status mf_align_depth_step(const float* prev_window, const float* cur_window, void* state, int W, int new_frames,
+                              int first_window, int height, int width, float* depth_out, void* stream);
+
 /* mf_motion_focus with the depth at the MODEL's resolution (the paper does not say how its depth
  * maps reach the focus-map resolution, reading F1 in DESIGN.md): depth_lowres is fp32 [count, depth_height, depth_width]
  * and is interpolated inside the render pass, bilinear with half-pixel centres and edge clamping (what

@@ -21,7 +21,8 @@ EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", 
            "mf_window_attention", "mf_chain_poses", "mf_motion_focus_workspace_size", "mf_motion_focus",
            "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
            "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step", "mf_motion_focus_upsampled",
-           "mf_align_depth_workspace_size", "mf_align_depth"]
+           "mf_align_depth_workspace_size", "mf_align_depth",
+           "mf_align_depth_state_size", "mf_align_depth_step"]
 
 
 class MfError(RuntimeError):
@@ -81,6 +82,8 @@ def lib():
         L.mf_align_depth_workspace_size.restype = ctypes.c_size_t
         L.mf_align_depth_workspace_size.argtypes = [ci]
         L.mf_align_depth.argtypes = [vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, ctypes.c_size_t, vp]
+        L.mf_align_depth_state_size.restype = ctypes.c_size_t
+        L.mf_align_depth_step.argtypes = [vp, vp, vp, ci, ci, ci, ci, ci, vp, vp]
         _lib = L
     return _lib
 
@@ -163,6 +166,25 @@ def align_depth(depth_local, stride, num_frames, workspace=None, out=None):
     _check(lib().mf_align_depth(_ptr(depth_local), nw, w, stride, num_frames, h, wd, _ptr(out), _ptr(scales), _ptr(workspace),
                                 workspace.numel(), _stream()))
     return out, scales
+
+
+def align_depth_state(device="cuda"):
+    """Device-resident state of the streaming depth alignment (mf_align_depth_step)."""
+    return torch.zeros((lib().mf_align_depth_state_size(),), device=device, dtype=torch.uint8)
+
+
+def align_depth_step(cur_window, state, prev_window=None, new_frames=0, first=False, out=None):
+    """One window [W, h, w] fp32 through the depth scale chain; returns the emitted frames fp32 [n, h, w]."""
+    _dev(cur_window, torch.float32, "cur_window")
+    if prev_window is not None:
+        _dev(prev_window, torch.float32, "prev_window")
+    w, h, wd = cur_window.shape
+    n = w if first else new_frames
+    if out is None:
+        out = torch.empty((max(n, 0), h, wd), device=cur_window.device, dtype=torch.float32)
+    _check(lib().mf_align_depth_step(_ptr(prev_window), _ptr(cur_window), _ptr(state), w, new_frames, 1 if first else 0, h, wd,
+                                     _ptr(out), _stream()))
+    return out
 
 
 def focus_params(n_points=15, sigma=20.0, vec=VEC_ACCEL, mag=MAG_UNIT, norm=NORM_MAX, pts=PTS_CURRENT_FRAME,

@@ -42,15 +42,10 @@ __device__ __forceinline__ void accumulate(float a, float b, double& sab, double
     }
 }
 
+// sum a b and sum b b over `count` floats (a: previous window, b: current), CTA blockIdx.y of kSumBlocks; out[2*blockIdx.y..]
 template <bool VEC>
-__global__ void __launch_bounds__(kSumThreads)
-overlap_sums_kernel(const float* __restrict__ depth_local, int W, int stride, int num_frames, size_t px,
-                    double* __restrict__ partials) {
-    const int n = blockIdx.x + 1;
-    const int s_prev = depth_win_start(n - 1, stride, num_frames, W), s_cur = depth_win_start(n, stride, num_frames, W);
-    const size_t count = static_cast<size_t>(s_prev + W - s_cur) * px;                 // shared frames x pixels
-    const float* a = depth_local + (static_cast<size_t>(n - 1) * W + (s_cur - s_prev)) * px;
-    const float* b = depth_local + static_cast<size_t>(n) * W * px;
+__device__ __forceinline__ void overlap_sums(const float* __restrict__ a, const float* __restrict__ b, size_t count,
+                                             double* __restrict__ out) {
     double sab = 0.0, sbb = 0.0;
     const size_t tid = static_cast<size_t>(blockIdx.y) * kSumThreads + threadIdx.x;
     const size_t nthreads = static_cast<size_t>(kSumBlocks) * kSumThreads;
@@ -102,8 +97,63 @@ overlap_sums_kernel(const float* __restrict__ depth_local, int W, int stride, in
             tab += s_ab[w];
             tbb += s_bb[w];
         }
-        partials[(static_cast<size_t>(n) * kSumBlocks + blockIdx.y) * 2] = tab;
-        partials[(static_cast<size_t>(n) * kSumBlocks + blockIdx.y) * 2 + 1] = tbb;
+        out[blockIdx.y * 2] = tab;
+        out[blockIdx.y * 2 + 1] = tbb;
+    }
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(kSumThreads)
+overlap_sums_kernel(const float* __restrict__ depth_local, int W, int stride, int num_frames, size_t px,
+                    double* __restrict__ partials) {
+    const int n = blockIdx.x + 1;
+    const int s_prev = depth_win_start(n - 1, stride, num_frames, W), s_cur = depth_win_start(n, stride, num_frames, W);
+    const size_t count = static_cast<size_t>(s_prev + W - s_cur) * px;                 // shared frames x pixels
+    overlap_sums<VEC>(depth_local + (static_cast<size_t>(n - 1) * W + (s_cur - s_prev)) * px,
+                      depth_local + static_cast<size_t>(n) * W * px, count, partials + static_cast<size_t>(n) * kSumBlocks * 2);
+}
+
+// Streaming form: one window pair per call, partials and the running scale in a small device-resident state.
+struct DepthState {
+    double c;                               // c_{n-1} before the call, c_n after it
+    double partials[kSumBlocks * 2];
+};
+
+template <bool VEC>
+__global__ void __launch_bounds__(kSumThreads)
+overlap_sums_step_kernel(const float* __restrict__ prev_shared, const float* __restrict__ cur, size_t count, DepthState* st) {
+    overlap_sums<VEC>(prev_shared, cur, count, st->partials);
+}
+
+__global__ void scale_step_kernel(DepthState* st, int first_window) {
+    if (first_window) {
+        st->c = 1.0;
+        return;
+    }
+    double sab = 0.0, sbb = 0.0;
+    for (int b = 0; b < kSumBlocks; ++b) {  // same fold order as scale_chain_kernel
+        sab += st->partials[b * 2];
+        sbb += st->partials[b * 2 + 1];
+    }
+    st->c *= sbb > 0.0 ? sab / sbb : 1.0;
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(kStitchThreads)
+stitch_step_kernel(const float* __restrict__ src_frames, const DepthState* __restrict__ st, size_t px, float* __restrict__ out) {
+    const double c = st->c;
+    const float* src = src_frames + static_cast<size_t>(blockIdx.x) * px;
+    float* dst = out + static_cast<size_t>(blockIdx.x) * px;
+    const size_t tid = static_cast<size_t>(blockIdx.y) * kStitchThreads + threadIdx.x;
+    const size_t nthreads = static_cast<size_t>(gridDim.y) * kStitchThreads;
+    auto scale1 = [c](float d) { return static_cast<float>(c * static_cast<double>(d)); };
+    if (VEC) {
+        for (size_t i = tid; i < (px >> 2); i += nthreads) {
+            const float4 d = ld_nc4(reinterpret_cast<const float4*>(src) + i);
+            st_cs4(reinterpret_cast<float4*>(dst) + i, make_float4(scale1(d.x), scale1(d.y), scale1(d.z), scale1(d.w)));
+        }
+    } else {
+        for (size_t i = tid; i < px; i += nthreads) dst[i] = scale1(__ldg(src + i));
     }
 }
 
@@ -201,6 +251,43 @@ extern "C" mf_status mf_align_depth(const float* depth_local, int num_windows, i
         stitch_kernel<true><<<sgrid, kStitchThreads, 0, q>>>(depth_local, scales, num_windows, W, stride, num_frames, px, depth_out);
     else
         stitch_kernel<false><<<sgrid, kStitchThreads, 0, q>>>(depth_local, scales, num_windows, W, stride, num_frames, px, depth_out);
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}
+
+extern "C" size_t mf_align_depth_state_size(void) { return sizeof(mf::DepthState); }
+
+extern "C" mf_status mf_align_depth_step(const float* prev_window, const float* cur_window, void* state, int W, int new_frames,
+                                         int first_window, int height, int width, float* depth_out, void* stream) {
+    using namespace mf;
+    if (!cur_window || !state || !depth_out) return fail(MF_ERR_INVALID_ARG, "mf_align_depth_step: NULL pointer");
+    if (reinterpret_cast<uintptr_t>(state) & 7u) return fail(MF_ERR_ALIGNMENT, "mf_align_depth_step: state must be 8-byte aligned");
+    if (W < 2 || width < 1 || height < 1) return fail(MF_ERR_INVALID_ARG, "mf_align_depth_step: bad sizes");
+    if (!first_window && (!prev_window || new_frames < 1 || new_frames >= W))
+        return fail(MF_ERR_INVALID_ARG, "mf_align_depth_step: need the previous window and 1 <= new_frames < W (got %d, W=%d)",
+                    new_frames, W);
+    if (mf_status s = require_sm100()) return s;
+    cudaStream_t q = static_cast<cudaStream_t>(stream);
+    DepthState* st = static_cast<DepthState*>(state);
+    const size_t px = static_cast<size_t>(height) * width;
+    const int emit = first_window ? W : new_frames;
+    const bool vec = (px % 4 == 0) && aligned16(cur_window) && aligned16(depth_out) && (first_window || aligned16(prev_window));
+    if (!first_window) {
+        const size_t count = static_cast<size_t>(W - new_frames) * px;
+        const float* a = prev_window + static_cast<size_t>(new_frames) * px;      // the frames both windows hold
+        if (vec)
+            overlap_sums_step_kernel<true><<<dim3(1, kSumBlocks), kSumThreads, 0, q>>>(a, cur_window, count, st);
+        else
+            overlap_sums_step_kernel<false><<<dim3(1, kSumBlocks), kSumThreads, 0, q>>>(a, cur_window, count, st);
+    }
+    scale_step_kernel<<<1, 1, 0, q>>>(st, first_window);
+    const size_t units = vec ? px / 4 : px;
+    const unsigned chunks = static_cast<unsigned>(std::min<size_t>((units + kStitchThreads * 4 - 1) / (kStitchThreads * 4), 1024));
+    const float* src = cur_window + static_cast<size_t>(W - emit) * px;
+    if (vec)
+        stitch_step_kernel<true><<<dim3(emit, chunks < 1 ? 1 : chunks), kStitchThreads, 0, q>>>(src, st, px, depth_out);
+    else
+        stitch_step_kernel<false><<<dim3(emit, chunks < 1 ? 1 : chunks), kStitchThreads, 0, q>>>(src, st, px, depth_out);
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
 }

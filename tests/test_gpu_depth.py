@@ -99,6 +99,28 @@ def test_align_depth_random_shapes(api, n, w, stride, h, wd, invalid, seed):
     _case(api, n, w, stride, h, wd, seed, invalid=invalid)
 
 
+@pytest.mark.parametrize("n,w,stride,h,wd", [(12, 4, 2, 6, 10), (13, 4, 2, 7, 9), (23, 8, 7, 5, 12), (9, 5, 1, 4, 4), (80, 32, 16, 74, 130)])
+def test_align_depth_step_reproduces_the_batch_call(api, n, w, stride, h, wd):
+    # streaming form: one window per call, scale carried in a device-resident state -> bit-identical to mf_align_depth
+    loc, _ = synth.depth_windows(n, w, stride, h, wd, 21 + n, invalid=0.05)
+    x = torch.from_numpy(loc).cuda()
+    ref, c_ref = api.align_depth(x, stride, n)
+    starts = ow.window_starts(n, w, stride)
+    state = api.align_depth_state()
+    parts = [api.align_depth_step(x[0], state, first=True)]
+    for i in range(1, len(starts)):
+        parts.append(api.align_depth_step(x[i], state, prev_window=x[i - 1], new_frames=starts[i] - starts[i - 1]))
+    got = torch.cat(parts)
+    assert got.shape == ref.shape
+    assert torch.equal(torch.nan_to_num(got, nan=-7.0), torch.nan_to_num(ref, nan=-7.0))
+    c_last = state[:8].view(torch.float64).item()
+    assert c_last == c_ref[-1].item()
+    with pytest.raises(api.MfError):
+        api.align_depth_step(x[1], state, prev_window=x[0], new_frames=w)        # new_frames must be < W
+    with pytest.raises(api.MfError):
+        api.align_depth_step(x[1], state, new_frames=1)                           # previous window required
+
+
 def test_align_depth_argument_errors(api):
     x = torch.ones((3, 4, 2, 2), device="cuda")
     with pytest.raises(api.MfError):
