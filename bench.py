@@ -306,7 +306,9 @@ def measure_streaming(wl, torch, api):
     """SURVEY 8(f) NEXT-2 (not part of the headline step): the path one window at a time, as a stream would see it.
     Per window: its q,k,v into static buffers, 24 attention launches, mf_chain_poses_step, the new poses appended to a
     rolling pose buffer, mf_motion_focus for the `stride` new frames.  Timed eagerly and as one replayed CUDA graph."""
+    from paper_2601_07154_b200 import synth
     c, dev = wl.cfg, wl.device
+    synth_seed = synth.seed_for(wl.cfg_idx, 9)
     m = wl.stride
     ring_len = wl.W + 32
     q, k, v = (torch.empty_like(t[:1]) for t in (wl.q, wl.k, wl.v))
@@ -405,6 +407,34 @@ def measure_streaming(wl, torch, api):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / len(windows)
 
+    # The same window step with the depth stream of Fig. 3: the window's model-resolution depth (518x294) is scale-aligned on the
+    # overlap (mf_align_depth_step), the new frames are emitted and the render interpolates them (mf_motion_focus_upsampled).
+    gd = torch.Generator(device=dev).manual_seed(synth_seed)
+    dwin = [torch.rand((wl.W, 294, 518), generator=gd, device=dev) * 29.0 + 1.0 for _ in range(2)]
+    dstate = api.align_depth_state(dev)
+    dnew = torch.empty((m, 294, 518), device=dev, dtype=torch.float32)
+    api.align_depth_step(dwin[0], dstate, first=True)
+
+    def step_depth():
+        attention()
+        api.chain_poses_step(win, state, new_frames=m, out=new)
+        ring.copy_(torch.cat([ring[m:], new]))
+        api.align_depth_step(dwin[1], dstate, prev_window=dwin[0], new_frames=m, out=dnew)
+        api.motion_focus_upsampled(ring, c["fx"], c["fy"], c["cx"], c["cy"], wl.width, wl.height, dnew, wl.params,
+                                   render_begin=ring_len - m, render_end=ring_len, workspace=ws,
+                                   out={"focus_map": fmap, "guided_depth": guided})
+
+    g_depth = torch.cuda.CUDAGraph()
+    side.wait_stream(main)
+    with torch.cuda.stream(side):
+        step_depth()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g_depth, stream=side):
+            step_depth()
+    main.wait_stream(side)
+    torch.cuda.synchronize()
+    depth_graph_ms = timed(g_depth.replay, range(5, 8))
+
     nwin = list(range(2, min(wl.Nw, 8)))
     back_to_back(run_overlapped, nwin[:2])
     serial_ms = back_to_back(run_serial, nwin)
@@ -413,6 +443,7 @@ def measure_streaming(wl, torch, api):
                     "mf_chain_poses_step + rolling pose buffer + mf_motion_focus of the new frames",
             "new_frames_per_window": m, "eager_ms_per_window": eager_ms, "graph_ms_per_window": graph_ms,
             "graph_back_to_back_ms_per_window": serial_ms, "two_stream_overlap_ms_per_window": overlap_ms,
+            "graph_ms_per_window_with_depth_alignment_and_upsampling": depth_graph_ms,
             "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
 
 
