@@ -121,6 +121,39 @@ def test_align_depth_step_reproduces_the_batch_call(api, n, w, stride, h, wd):
         api.align_depth_step(x[1], state, new_frames=1)                           # previous window required
 
 
+def test_streaming_depth_pipeline_matches_batch(api):
+    # per window: chain step -> rolling pose buffer, depth scale step -> new frames, render with in-pass upsampling
+    # == chain_poses + align_depth + motion_focus_upsampled on the whole clip, bit for bit
+    cfg = synth.CONFIGS[1]
+    n_frames, w, stride = 48, 8, 4
+    width, height, k = 256, 128, (180.0, 180.0, 128.0, 64.0)
+    traj = synth.trajectory(cfg, synth.seed_for(1, 21), n_frames)
+    loc = torch.from_numpy(synth.local_windows(traj, w, stride, seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
+    dloc = torch.from_numpy(synth.depth_windows(n_frames, w, stride, 36, 64, 31)[0]).cuda()
+    prm = api.focus_params(n_points=15, sigma=12.0)
+    poses = api.chain_poses(loc, stride, n_frames)
+    stream, _ = api.align_depth(dloc, stride, n_frames)
+    batch = api.motion_focus_upsampled(poses, *k, width, height, stream, prm)
+    ring_len = w + 24
+    ring = torch.zeros((ring_len, 4, 4), device="cuda", dtype=torch.float64)
+    pstate, dstate = api.chain_state(), api.align_depth_state()
+    t_done = 0
+    for n in range(loc.shape[0]):
+        new = api.chain_poses_step(loc[n], pstate, new_frames=stride, first=n == 0)
+        dnew = api.align_depth_step(dloc[n], dstate, prev_window=dloc[n - 1] if n else None, new_frames=stride, first=n == 0)
+        m = new.shape[0]
+        assert dnew.shape[0] == m and torch.equal(dnew, stream[t_done:t_done + m])
+        ring = torch.cat([ring[m:], new])
+        t_done += m
+        if t_done < ring_len:
+            continue
+        out = api.motion_focus_upsampled(ring, *k, width, height, dnew, prm, render_begin=ring_len - m, render_end=ring_len)
+        sl = slice(t_done - m, t_done)
+        assert torch.equal(out["focus_index"], batch["focus_index"][sl])
+        assert torch.equal(out["focus_map"], batch["focus_map"][sl]) and torch.equal(out["guided_depth"], batch["guided_depth"][sl])
+    assert t_done == n_frames
+
+
 def test_align_depth_argument_errors(api):
     x = torch.ones((3, 4, 2, 2), device="cuda")
     with pytest.raises(api.MfError):
