@@ -118,7 +118,7 @@ def test_suburban_window_sampled_rows(api):
     _check(api, 2, w, p, 16, oa.FRAME, synth.seed_for(1, 0), rows=rows, lse=True)
 
 
-def _a7_rows(w, p, seed, n_random=256, edge=64):
+def _a7_rows(w, p, seed, n_random=512, edge=128):
     """Reading A7: seeded random rows + the first and last rows + the rows next to every frame boundary."""
     rng = np.random.default_rng(seed)
     s_len = w * p
