@@ -302,6 +302,29 @@ def measure_d128(wl, torch, api, peak_sustained):
             "frac_of_sustained_peak": tf / peak_sustained}
 
 
+def measure_one_wave(wl, torch, api, peak_sustained):
+    """the tiny config is launch-bound at one window, so its GLOBAL layer is also timed with 148 windows per launch
+    (one window-head per SM and q-block wave)."""
+    from paper_2601_07154_b200 import synth
+    nw = 148
+    q, k, v = synth.qkv(nw, wl.S, wl.H, wl.D, synth.seed_for(wl.cfg_idx, 10), device=wl.device)
+    o = torch.empty_like(q)
+    for _ in range(3):
+        api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+    torch.cuda.synchronize()
+    n = 100
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n):
+        api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / n
+    tf = wl.flops_global * nw / (ms * 1e-3) / 1e12
+    return {"what": "GLOBAL layer of this config with 148 windows per launch (SURVEY 8(d))", "windows_per_launch": nw,
+            "us_per_launch": ms * 1e3, "tflops": tf, "frac_of_sustained_peak": tf / peak_sustained}
+
+
 def measure_streaming(wl, torch, api):
     """SURVEY 8(f) NEXT-2 (not part of the headline step): the path one window at a time, as a stream would see it.
     Per window: its q,k,v into static buffers, 24 attention launches, mf_chain_poses_step, the new poses appended to a
@@ -625,6 +648,10 @@ def main():
     if rank == 0 and not args.no_d128 and wl.D == 64:
         d128 = measure_d128(wl, torch, api, peaks["tf_sustained"])
 
+    one_wave = None
+    if rank == 0 and wl.S <= 2048:
+        one_wave = measure_one_wave(wl, torch, api, peaks["tf_sustained"])
+
     streaming = None
     if rank == 0 and not args.no_stream and wl.Nw >= 8 and wl.layers > 1:
         streaming = measure_streaming(wl, torch, api)
@@ -636,7 +663,7 @@ def main():
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
                 "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
-                "cpu_baseline": cpu, "e2e": e2e, "block": block, "head_dim_128": d128, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+                "cpu_baseline": cpu, "e2e": e2e, "block": block, "head_dim_128": d128, "windows_148": one_wave, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
         print(json.dumps(line))
     replicas.finish()
 

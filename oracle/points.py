@@ -82,6 +82,7 @@ def motion_points(global_w2c, fx, fy, cx, cy, width, height, n_points, sigma,
                    oldest first)
       focus_uv     (np.float32 u, np.float32 v) of the frame's own point, NaN if invalid
       focus_index  int, y*width + x, or -1
+      focus_uv64   the same point before rounding to fp32 (Python floats), None if invalid
     """
     sigma = float(np.float32(sigma))                      # the API carries sigma as fp32
     poses = [from_4x4(m) for m in global_w2c]
@@ -108,5 +109,6 @@ def motion_points(global_w2c, fx, fy, cx, cy, width, height, n_points, sigma,
             x = math.floor(own[0] + 0.5) if math.isfinite(own[0]) else -1
             y = math.floor(own[1] + 0.5) if math.isfinite(own[1]) else -1
             index = y * width + x if (0 <= x < width and 0 <= y < height) else -1
-        frames.append({"points": pts_t, "focus_uv": uv, "focus_index": index})
+        frames.append({"points": pts_t, "focus_uv": uv, "focus_index": index,
+                       "focus_uv64": None if own is None else (own[0], own[1])})    # unrounded (u, v): near-tie reports only
     return frames
