@@ -157,13 +157,15 @@ def test_tiny_config_focus(api):
     assert abs(fm[2].max() - 1.0) < 1e-6 and abs(fm[3].max() - 1.0) < 1e-6
 
 
-@pytest.mark.parametrize("cfg_idx,n_frames,rb,re_", [(1, 40, 0, 40), (2, 30, 22, 28), (3, 30, 25, 29), (4, 20, 18, 20)])
-def test_config_shaped_focus(api, cfg_idx, n_frames, rb, re_):
+@pytest.mark.parametrize("cfg_idx,n_frames,rb,re_,sigma", [(1, 40, 0, 40, None), (2, 30, 22, 28, None), (3, 30, 25, 29, None),
+                                                          (4, 20, 18, 20, None),
+                                                          (4, 20, 19, 20, 40.0)])   # S8(d): town also at sigma = 40 px
+def test_config_shaped_focus(api, cfg_idx, n_frames, rb, re_, sigma):
     cfg = synth.CONFIGS[cfg_idx]
     poses = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
     depth = synth.depth(re_ - rb, cfg["height"], cfg["width"], synth.seed_for(cfg_idx, 3)).numpy()
     worst, _, _ = _focus_case(api, poses, (cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"]), cfg["width"], cfg["height"],
-                              depth, render_begin=rb, render_end=re_, sigma=cfg["sigma"])
+                              depth, render_begin=rb, render_end=re_, sigma=cfg["sigma"] if sigma is None else sigma)
     assert worst <= 1.0, worst
 
 
