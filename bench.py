@@ -470,6 +470,17 @@ def measure_streaming(wl, torch, api):
             "frames_per_s_streaming": m / (graph_ms * 1e-3), "kernels_per_window": wl.layers + 1 + 3}
 
 
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def oracle_sample(cfg_idx, wl_dims, rows=4096):
     """Times the oracle, as it stands, on a bounded sample of the same workload (host cores) and
     extrapolates to the whole clip.  Returns (frames_per_s, seconds_of_sample, description, cores)."""
@@ -638,7 +649,8 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dims = dims_of(args.config, args)
         fps, secs, desc, cores = oracle_sample(args.config, dims)
-        cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc, "sample_seconds": secs}
+        cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc, "sample_seconds": secs,
+               "cpu_model": cpu_model(), "nproc": os.cpu_count()}
 
     block = None
     if rank == 0 and not args.no_block and wl.layers > 1:
