@@ -119,7 +119,7 @@ class Workload:
         self.S = self.W * self.P
         self.stride, self.layers = cfg["stride"], cfg["layers"]
         self.N = cfg["N"]
-        self.Nw = synth.num_windows(self.N, self.W, self.stride)
+        self.Nw = api.num_windows(self.N, self.W, self.stride)
         if args.max_windows and args.max_windows < self.Nw:
             self.Nw = args.max_windows
             self.N = (self.Nw - 1) * self.stride + self.W
@@ -142,7 +142,7 @@ class Workload:
         self.q, self.k, self.v = synth.qkv(self.Nw, self.S, self.H, self.D, synth.seed_for(self.cfg_idx, 0), device=dev)
         self.o = [torch.empty((self.B, self.S, self.H, self.D), device=dev, dtype=torch.bfloat16) for _ in range(2)]
         traj = synth.trajectory(self.cfg, synth.seed_for(self.cfg_idx, 1), self.N)
-        self.local_np = synth.local_windows(traj, self.W, self.stride, seed=synth.seed_for(self.cfg_idx, 2),
+        self.local_np = synth.local_windows(traj, self.W, api.window_starts(self.N, self.W, self.stride), seed=synth.seed_for(self.cfg_idx, 2),
                                             perturb_rot=1e-3, perturb_t=1e-3)
         self.local = torch.from_numpy(self.local_np).to(dev)
         self.depth = synth.depth(self.N, self.height, self.width, synth.seed_for(self.cfg_idx, 3), device=dev)
@@ -491,6 +491,7 @@ def oracle_sample(cfg_idx, wl_dims, rows=4096):
     from oracle import chain as oc
     from oracle import points as op
     from oracle import render as orr
+    from oracle import windows as ow
     from paper_2601_07154_b200 import synth
     cfg = synth.CONFIGS[cfg_idx]
     W, P, H, D, S, Nw, N, layers = (wl_dims[k] for k in ("W", "P", "H", "D", "S", "Nw", "N", "layers"))
@@ -504,7 +505,7 @@ def oracle_sample(cfg_idx, wl_dims, rows=4096):
     oa.window_attention(q, k, v, W, P, oa.FRAME, rows=np.arange(P))
     t_frame = time.perf_counter() - t0
     traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), N)
-    loc = synth.local_windows(traj, W, cfg["stride"], seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    loc = synth.local_windows(traj, W, ow.window_starts(N, W, cfg["stride"]), seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
     t0 = time.perf_counter()
     poses = oc.chain_poses(loc.tolist(), W, cfg["stride"], N)
     frames = op.motion_points(poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"], 15, cfg["sigma"])
@@ -524,10 +525,11 @@ def oracle_sample(cfg_idx, wl_dims, rows=4096):
     return N / total, t_global + t_frame + t_pose + t_render, desc, min(cores, blas) if blas > 1 else 1
 
 
-def dims_of(cfg_idx, args):
+def dims_of(cfg_idx, args, num_windows):
+    """num_windows: the caller's window count (the library's mf_num_windows for our arm, oracle/windows.py for the reference arm)."""
     from paper_2601_07154_b200 import synth
     c = synth.CONFIGS[cfg_idx]
-    nw = synth.num_windows(c["N"], c["W"], c["stride"])
+    nw = num_windows(c["N"], c["W"], c["stride"])
     n = c["N"]
     if args.max_windows and args.max_windows < nw:
         nw = args.max_windows
@@ -553,7 +555,8 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    dims = dims_of(args.config, args)
+    from oracle import windows as ow
+    dims = dims_of(args.config, args, ow.num_windows)
     vals, secs, desc, cores = [], [], "", 1
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()
@@ -647,7 +650,7 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        dims = dims_of(args.config, args)
+        dims = dims_of(args.config, args, api.num_windows)
         fps, secs, desc, cores = oracle_sample(args.config, dims)
         cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": desc, "sample_seconds": secs,
                "cpu_model": cpu_model(), "nproc": os.cpu_count()}
@@ -669,7 +672,7 @@ def main():
         streaming = measure_streaming(wl, torch, api)
 
     if rank == 0:
-        dims = dims_of(args.config, args)
+        dims = dims_of(args.config, args, api.num_windows)
         line = {"metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)", "value": value,
                 "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",

@@ -116,6 +116,15 @@ def window_start(num_frames, w, stride, n):
     return lib().mf_window_start(num_frames, w, stride, n)
 
 
+def window_starts(num_frames, w, stride):
+    """[mf_window_start(n) for every window] (host arithmetic of the library, no device needed)."""
+    L = lib()
+    nw = L.mf_num_windows(num_frames, w, stride)
+    if nw < 0:
+        raise MfError("window_starts: need num_frames >= W > stride >= 1")
+    return [L.mf_window_start(num_frames, w, stride, n) for n in range(nw)]
+
+
 def window_attention(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLOBAL, softmax_scale=0.0,
                      out=None, return_lse=False):
     """q,k,v: bf16 CUDA [windows, S, H, D] with S = frames_per_window*tokens_per_frame."""

@@ -43,14 +43,6 @@ def seed_for(config_index, stream):
     return BASE_SEED + 1000 * config_index + stream
 
 
-def num_windows(n, w, stride):
-    return -(-(n - w) // stride) + 1
-
-
-def window_starts(n, w, stride):
-    return [min(i * stride, n - w) for i in range(num_windows(n, w, stride))]
-
-
 def qkv(windows, s_len, heads, dim, seed, device="cpu", scale=1.0):
     """Three bf16 tensors [windows, S, H, D] ~ N(0, scale^2), seeded."""
     import torch
@@ -104,15 +96,18 @@ def trajectory(cfg, seed, num_frames=None):
     return out
 
 
-def local_windows(global_w2c, w, stride, seed=None, perturb_rot=0.0, perturb_t=0.0):
-    """Cut a trajectory into window-local poses, fp32 [Nw, W, 4, 4].
+def local_windows(global_w2c, w, starts, seed=None, perturb_rot=0.0, perturb_t=0.0):
+    """Cut a trajectory into window-local poses, fp32 [len(starts), W, 4, 4].
+
+    `starts` = the first frame of every window.  The caller supplies it (the window partition is step a1 of the
+    method: tests take it from oracle/windows.py, bench.py and smoke() from mf_window_start), so this
+    module holds none of the method's arithmetic.
 
     Window n's local world is its own first camera (6-DoF gauge).  Optional
     per-frame perturbation makes overlapping estimates disagree like a real
     model's would.
     """
-    n = global_w2c.shape[0]
-    starts = window_starts(n, w, stride)
+    starts = list(starts)
     rng = np.random.default_rng(seed)
     out = np.zeros((len(starts), w, 4, 4), dtype=np.float32)
     for i, s0 in enumerate(starts):
@@ -138,14 +133,15 @@ def depth(frames, height, width, seed, device="cpu"):
                       dtype=torch.float32) * 29.0 + 1.0
 
 
-def depth_windows(num_frames, w, stride, height, width, seed, gauge_spread=2.0, noise=0.02, invalid=0.0):
-    """Window-local depth maps, fp32 numpy [Nw, W, height, width]: one Uniform(1, 30) m stream, cut into windows, each window
+def depth_windows(num_frames, w, starts, height, width, seed, gauge_spread=2.0, noise=0.02, invalid=0.0):
+    """Window-local depth maps, fp32 numpy [Nw, W, height, width]: one Uniform(1, 30) m stream, cut into windows at the
+    caller-supplied `starts` (see local_windows), each window
     divided by its own scale (log-uniform in [1/gauge_spread, gauge_spread]) and multiplied by per-pixel noise
     (1 + noise * N(0,1)), so that overlapping estimates disagree like a model's would.  A fraction `invalid` of the pixels is
     replaced by 0, NaN or inf (sky / holes).  Returns (depth_local, gauges)."""
     rng = np.random.default_rng(seed)
     stream = rng.uniform(1.0, 30.0, (num_frames, height, width))
-    starts = window_starts(num_frames, w, stride)
+    starts = list(starts)
     gauges = np.exp(rng.uniform(-np.log(gauge_spread), np.log(gauge_spread), len(starts)))
     out = np.empty((len(starts), w, height, width), dtype=np.float32)
     for i, s0 in enumerate(starts):

@@ -8,6 +8,7 @@ import torch
 from oracle import chain as oc
 from oracle import points as op
 from oracle import render as orr
+from oracle import windows as ow
 from paper_2601_07154_b200 import synth
 
 pytestmark = pytest.mark.gpu
@@ -25,7 +26,7 @@ def _chain_case(api, cfg_idx, n_frames, mode, perturb=True, w=None, stride=None)
     w = cfg["W"] if w is None else w
     stride = cfg["stride"] if stride is None else stride
     traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
-    loc = synth.local_windows(traj, w, stride, seed=synth.seed_for(cfg_idx, 2),
+    loc = synth.local_windows(traj, w, ow.window_starts(len(traj), w, stride), seed=synth.seed_for(cfg_idx, 2),
                               perturb_rot=1e-3 if perturb else 0.0, perturb_t=1e-3 if perturb else 0.0)
     ref = np.array(oc.chain_poses(loc.tolist(), w, stride, n_frames, mode))
     got = api.chain_poses(torch.from_numpy(loc).cuda(), stride, n_frames, mode).cpu().numpy()
@@ -46,10 +47,9 @@ def test_chain_bit_exact(api, cfg_idx, n_frames, w, stride, mode):
 @pytest.mark.parametrize("cfg_idx,n_frames,w,stride", [(3, 200, 32, 16), (1, 23, 8, 7), (1, 9, 4, 1), (4, 720, 64, 32)])
 def test_chain_streaming_matches_batch_bit_for_bit(api, cfg_idx, n_frames, w, stride, mode):
     # mf_chain_poses_step ("incremental"): one window per call, state carried on the device
-    from oracle import windows as ow
     cfg = synth.CONFIGS[cfg_idx]
     traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), n_frames)
-    loc = synth.local_windows(traj, w, stride, seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    loc = synth.local_windows(traj, w, ow.window_starts(len(traj), w, stride), seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
     ref = np.array(oc.chain_poses(loc.tolist(), w, stride, n_frames, mode))
     dloc = torch.from_numpy(loc).cuda()
     state = api.chain_state()
@@ -71,7 +71,7 @@ def test_streaming_pipeline_matches_batch(api):
     width, height = 256, 128
     k = (180.0, 180.0, 128.0, 64.0)
     traj = synth.trajectory(cfg, synth.seed_for(1, 21), n_frames)
-    loc = torch.from_numpy(synth.local_windows(traj, w, stride, seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
+    loc = torch.from_numpy(synth.local_windows(traj, w, ow.window_starts(len(traj), w, stride), seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
     depth = synth.depth(n_frames, height, width, 77, device="cuda")
     prm = api.focus_params(n_points=n_points, sigma=12.0)
     poses = api.chain_poses(loc, stride, n_frames)
@@ -98,7 +98,7 @@ def test_streaming_pipeline_matches_batch(api):
 def test_chain_multi_sequence_and_errors(api):
     cfg = synth.CONFIGS[1]
     traj = [synth.trajectory(cfg, synth.seed_for(1, 10 + i), 40) for i in range(3)]
-    loc = np.stack([synth.local_windows(t, 8, 4, seed=i, perturb_rot=1e-3, perturb_t=1e-3) for i, t in enumerate(traj)])
+    loc = np.stack([synth.local_windows(t, 8, ow.window_starts(len(t), 8, 4), seed=i, perturb_rot=1e-3, perturb_t=1e-3) for i, t in enumerate(traj)])
     got = api.chain_poses(torch.from_numpy(loc).cuda(), 4, 40).cpu().numpy()
     for i in range(3):
         assert np.array_equal(got[i], np.array(oc.chain_poses(loc[i].tolist(), 8, 4, 40)))
@@ -186,7 +186,7 @@ def test_focus_chain_to_focus_pipeline_bit_exact_index(api):
     cfg = synth.CONFIGS[2]
     n = 200
     traj = synth.trajectory(cfg, synth.seed_for(2, 1), n)
-    loc = synth.local_windows(traj, 16, 8, seed=synth.seed_for(2, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    loc = synth.local_windows(traj, 16, ow.window_starts(len(traj), 16, 8), seed=synth.seed_for(2, 2), perturb_rot=1e-3, perturb_t=1e-3)
     ref_poses = oc.chain_poses(loc.tolist(), 16, 8, n)
     g = api.chain_poses(torch.from_numpy(loc).cuda(), 8, n)
     prm = api.focus_params(n_points=15, sigma=20.0)

@@ -21,7 +21,7 @@ def api():
 
 
 def _case(api, n, w, stride, h, wd, seed, **kw):
-    loc, _ = synth.depth_windows(n, w, stride, h, wd, seed, **kw)
+    loc, _ = synth.depth_windows(n, w, ow.window_starts(n, w, stride), h, wd, seed, **kw)
     ref, c_ref = od.align_depth(loc, w, stride, n)
     got, c = api.align_depth(torch.from_numpy(loc).cuda(), stride, n)
     torch.cuda.synchronize()
@@ -49,7 +49,7 @@ def test_align_depth_parity(api, n, w, stride, h, wd):
 
 def test_align_depth_recovers_gauges_and_ignores_invalid_pixels(api):
     n, w, stride = 40, 8, 4
-    loc, g = synth.depth_windows(n, w, stride, 16, 20, 5, noise=0.0)
+    loc, g = synth.depth_windows(n, w, ow.window_starts(n, w, stride), 16, 20, 5, noise=0.0)
     got, c = api.align_depth(torch.from_numpy(loc).cuda(), stride, n)
     assert np.abs(c.cpu().numpy() - g / g[0]).max() <= 1e-6        # fp32 inputs: the gauges come back to fp32 accuracy
     _case(api, n, w, stride, 16, 20, 6, invalid=0.2)               # zeros, NaN, inf, negatives in both windows
@@ -65,7 +65,7 @@ def test_align_depth_recovers_gauges_and_ignores_invalid_pixels(api):
 
 def test_align_depth_is_deterministic_and_feeds_the_focus_call(api):
     n, w, stride, h, wd = 48, 32, 16, 294, 518
-    loc, _ = synth.depth_windows(n, w, stride, h, wd, 3)
+    loc, _ = synth.depth_windows(n, w, ow.window_starts(n, w, stride), h, wd, 3)
     x = torch.from_numpy(loc).cuda()
     a, ca = api.align_depth(x, stride, n)
     b, cb = api.align_depth(x, stride, n)
@@ -102,7 +102,7 @@ def test_align_depth_random_shapes(api, n, w, stride, h, wd, invalid, seed):
 @pytest.mark.parametrize("n,w,stride,h,wd", [(12, 4, 2, 6, 10), (13, 4, 2, 7, 9), (23, 8, 7, 5, 12), (9, 5, 1, 4, 4), (80, 32, 16, 74, 130)])
 def test_align_depth_step_reproduces_the_batch_call(api, n, w, stride, h, wd):
     # streaming form: one window per call, scale carried in a device-resident state -> bit-identical to mf_align_depth
-    loc, _ = synth.depth_windows(n, w, stride, h, wd, 21 + n, invalid=0.05)
+    loc, _ = synth.depth_windows(n, w, ow.window_starts(n, w, stride), h, wd, 21 + n, invalid=0.05)
     x = torch.from_numpy(loc).cuda()
     ref, c_ref = api.align_depth(x, stride, n)
     starts = ow.window_starts(n, w, stride)
@@ -128,8 +128,8 @@ def test_streaming_depth_pipeline_matches_batch(api):
     n_frames, w, stride = 48, 8, 4
     width, height, k = 256, 128, (180.0, 180.0, 128.0, 64.0)
     traj = synth.trajectory(cfg, synth.seed_for(1, 21), n_frames)
-    loc = torch.from_numpy(synth.local_windows(traj, w, stride, seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
-    dloc = torch.from_numpy(synth.depth_windows(n_frames, w, stride, 36, 64, 31)[0]).cuda()
+    loc = torch.from_numpy(synth.local_windows(traj, w, ow.window_starts(n_frames, w, stride), seed=5, perturb_rot=1e-3, perturb_t=1e-3)).cuda()
+    dloc = torch.from_numpy(synth.depth_windows(n_frames, w, ow.window_starts(n_frames, w, stride), 36, 64, 31)[0]).cuda()
     prm = api.focus_params(n_points=15, sigma=12.0)
     poses = api.chain_poses(loc, stride, n_frames)
     stream, _ = api.align_depth(dloc, stride, n_frames)

@@ -14,6 +14,7 @@ def _free_port():
 def _worker(rank, world, port, out):
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
                       MASTER_PORT=str(port))
+    from oracle import windows as ow
     from paper_2601_07154_b200 import replicas, synth
     assert replicas.init("gloo") == world
     assert replicas.env_world() == (rank, rank, world)
@@ -24,7 +25,7 @@ def _worker(rank, world, port, out):
     # every rank builds the same seeded clip (replicas): identical window partition and local poses on all ranks
     cfg = synth.CONFIGS[1]
     traj = synth.trajectory(cfg, synth.seed_for(1, 1), 24)
-    loc = synth.local_windows(traj, cfg["W"], cfg["stride"], seed=synth.seed_for(1, 2))
+    loc = synth.local_windows(traj, cfg["W"], ow.window_starts(len(traj), cfg["W"], cfg["stride"]), seed=synth.seed_for(1, 2))
     checksum = replicas.max_over_ranks(float(abs(loc).sum())) - float(abs(loc).sum())
     replicas.barrier()
     out.put((rank, ms, value, checksum))
