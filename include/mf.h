@@ -8,7 +8,11 @@
  *    The library never frees or retains caller memory.
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued
  *    on it and the call returns without synchronising (the *_host variants synchronise).
- *  - Return value is an mf_status.  On any error nothing has been enqueued.
+ *  - Return value is an mf_status.  Every argument, shape, alignment, workspace and device check is made
+ *    before the first enqueue (the *_host variants run the checks of every call they are about to make before
+ *    they allocate or copy), so MF_ERR_INVALID_ARG / UNSUPPORTED / ALIGNMENT / WORKSPACE mean nothing has been
+ *    enqueued.  MF_ERR_CUDA reports a failing CUDA runtime call (allocation, copy, launch); work the same call
+ *    enqueued before that failure may still run.
  *    mf_last_error() returns a thread-local, human-readable message for the last failure.
  *  - No CPU fallback: a device that is not sm_100, an unsupported shape or a misaligned
  *    pointer is an error.  NaN/Inf in inputs are not checked (they propagate).
@@ -107,7 +111,8 @@ mf_status mf_chain_poses_step(const float* window_local_w2c, void* state, int W,
  *   Eq.1  p_t = -R_t^T t_t                       Eq.3  a_w = p_i - 2 p_{i-1} + p_{i-2}
  *   Eq.4  a_c = R a_w                            Eq.6  (u,v) = (cx + fx ax/az, cy + fy ay/az)
  *   Eq.7  M(x,y) = (1/Z) sum_{i in trailing n_points frames} exp(-((x-u_i)^2+(y-v_i)^2)/(2 sigma_i^2))
- *   G(x,y) = M(x,y) * depth(x,y)
+ *   G(x,y) = M(x,y) * depth(x,y), and G = 0 exactly wherever M = 0 whatever depth holds there (a NaN/Inf depth
+ *   sample propagates only inside the map's support; reading G1 in DESIGN.md).  The depth is not read where M = 0.
  * Pixel (x,y) is centred at (u,v) = (x,y).  A point is skipped when it needs a frame < 0,
  * when |a_w| < 1e-12, or when |a_z| <= eps_z*|a_c|.  sigma_i = sigma*|a_w| (MF_MAG_RAW) or
  * sigma (MF_MAG_UNIT), clamped to >= 1e-3 px.  Z = per-frame max over pixels (MF_NORM_MAX),

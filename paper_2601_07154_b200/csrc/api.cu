@@ -1,6 +1,7 @@
 // Status strings, error buffer, device check and window arithmetic of the mf C ABI (include/mf.h).
 #include "common.h"
 
+#include <atomic>
 #include <cstring>
 
 namespace mf {
@@ -18,26 +19,38 @@ mf_status fail(mf_status s, const char* fmt, ...) {
     return s;
 }
 
-static int g_checked_device = -1;
-static int g_sm_count = 0;
+bool& validate_only() {
+    static thread_local bool flag = false;
+    return flag;
+}
+
+// SM count of every device that passed the check (0 = not checked yet).  The library is called from several host
+// threads at once (bench.py's end-to-end path), so the cache is one atomic per device, written after the check.
+constexpr int kMaxDevices = 64;
+static std::atomic<int> g_sm_count[kMaxDevices];
 
 mf_status require_sm100() {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail(MF_ERR_CUDA, "cudaGetDevice failed: %s", cudaGetErrorString(e));
-    if (dev == g_checked_device) return MF_OK;
-    cudaDeviceProp prop;
-    e = cudaGetDeviceProperties(&prop, dev);
-    if (e != cudaSuccess) return fail(MF_ERR_CUDA, "cudaGetDeviceProperties failed: %s", cudaGetErrorString(e));
-    if (prop.major != 10)
-        return fail(MF_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only (no fallback)",
-                    dev, prop.major, prop.minor);
-    g_sm_count = prop.multiProcessorCount;
-    g_checked_device = dev;
+    if (dev >= 0 && dev < kMaxDevices && g_sm_count[dev].load(std::memory_order_acquire) > 0) return MF_OK;
+    int major = 0, minor = 0, sms = 0;
+    if ((e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+        return fail(MF_ERR_CUDA, "cudaDeviceGetAttribute failed: %s", cudaGetErrorString(e));
+    if (major != 10)
+        return fail(MF_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only (no fallback)", dev, major, minor);
+    if (dev >= 0 && dev < kMaxDevices) g_sm_count[dev].store(sms > 0 ? sms : 148, std::memory_order_release);
     return MF_OK;
 }
 
-int sm_count() { return g_sm_count > 0 ? g_sm_count : 148; }
+int sm_count() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return 148;
+    const int n = g_sm_count[dev].load(std::memory_order_acquire);
+    return n > 0 ? n : 148;
+}
 
 }  // namespace mf
 

@@ -1,8 +1,12 @@
-// Host-buffer entry points (end-to-end path): allocate device buffers from the stream-ordered pool,
-// copy in, run the device entry points, copy out, synchronise.  See include/mf.h.
+// Host-buffer entry points (end-to-end path): validate the whole chain of device calls first (mf::validate_only), then
+// allocate device buffers from the stream-ordered pool, copy in, run the device entry points, copy out, synchronise.
+// See include/mf.h.
 #include "common.h"
 
 namespace {
+
+// Fake, distinct, 16-byte aligned device addresses for the validation pass (never dereferenced).
+inline void* fake(int i) { return reinterpret_cast<void*>(static_cast<uintptr_t>(0x1000) * (i + 1)); }
 
 struct DeviceBuf {
     void* p = nullptr;
@@ -25,6 +29,15 @@ extern "C" mf_status mf_window_attention_host(const void* q, const void* k, cons
         return mf::fail(MF_ERR_INVALID_ARG, "mf_window_attention_host: non-positive dimension");
     if (first_mode != MF_ATTN_GLOBAL && first_mode != MF_ATTN_FRAME)
         return mf::fail(MF_ERR_INVALID_ARG, "mf_window_attention_host: bad mode");
+    {   // everything the per-layer calls below would reject, before anything is allocated or copied
+        mf::ValidateOnlyScope dry;
+        for (int l = 0; l < (num_layers > 1 ? 2 : 1); ++l) {
+            const mf_attn_mode m = (l % 2 == 0) ? first_mode : (first_mode == MF_ATTN_GLOBAL ? MF_ATTN_FRAME : MF_ATTN_GLOBAL);
+            mf_status st = mf_window_attention(fake(0), fake(1), fake(2), fake(3), nullptr, windows, frames_per_window,
+                                               tokens_per_frame, heads, head_dim, m, softmax_scale, stream);
+            if (st != MF_OK) return st;
+        }
+    }
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t bytes = static_cast<size_t>(windows) * frames_per_window * tokens_per_frame * heads * head_dim * 2;
     DeviceBuf dq(s), dk(s), dv(s), dout(s), dout2(s);
@@ -64,6 +77,17 @@ extern "C" mf_status mf_chain_and_focus_host(const float* local_w2c, int num_win
     const size_t img_bytes = static_cast<size_t>(count) * width * height * sizeof(float);
     const size_t ws_bytes = mf_motion_focus_workspace_size(count, width, height, params->n_points);
     if (ws_bytes == 0) return mf::fail(MF_ERR_INVALID_ARG, "mf_chain_and_focus_host: bad n_points or image size");
+    {   // everything mf_chain_poses / mf_motion_focus below would reject, before anything is allocated or copied
+        mf::ValidateOnlyScope dry;
+        mf_status st = mf_chain_poses(static_cast<const float*>(fake(0)), 1, num_windows, W, stride, num_frames, align,
+                                      static_cast<double*>(fake(1)), stream);
+        if (st != MF_OK) return st;
+        st = mf_motion_focus(static_cast<const double*>(fake(1)), K, num_frames, render_begin, render_end, width, height,
+                             depth ? static_cast<const float*>(fake(2)) : nullptr, params,
+                             focus_map ? static_cast<float*>(fake(3)) : nullptr, guided_depth ? static_cast<float*>(fake(4)) : nullptr,
+                             static_cast<float*>(fake(5)), static_cast<int32_t*>(fake(6)), fake(7), ws_bytes, stream);
+        if (st != MF_OK) return st;
+    }
     DeviceBuf dloc(s), dpose(s), ddepth(s), dmap(s), dg(s), duv(s), didx(s), dws(s);
     MF_CUDA_OK(dloc.alloc(loc_bytes));
     MF_CUDA_OK(dpose.alloc(pose_bytes));

@@ -380,6 +380,9 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if (seq_len_ll > (1 << 24) || sequences_ll > (1 << 24))
         return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: sequence length / count too large");
     const int sequences = static_cast<int>(sequences_ll), seq_len = static_cast<int>(seq_len_ll);
+    if (static_cast<long long>((seq_len + 255) / 256) * heads * sequences > 0x7fffffffLL)
+        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
+    if (validate_only()) return MF_OK;
 
     AttnParams prm;
     prm.seq_len = seq_len;

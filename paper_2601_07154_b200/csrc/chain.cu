@@ -191,6 +191,7 @@ extern "C" mf_status mf_chain_poses(const float* local_w2c, int sequences, int n
     if (smem > 200 * 1024)
         return mf::fail(MF_ERR_UNSUPPORTED, "mf_chain_poses: num_windows=%d exceeds the on-chip fold buffer (max 2133)",
                         num_windows);
+    if (mf::validate_only()) return MF_OK;
     if (smem > 48 * 1024)
         MF_CUDA_OK(cudaFuncSetAttribute(mf::chain_poses_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         static_cast<int>(smem)));

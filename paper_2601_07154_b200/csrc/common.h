@@ -13,9 +13,19 @@ namespace mf {
 char* error_buffer();
 mf_status fail(mf_status s, const char* fmt, ...);
 
-// Checks that the current device is an sm_100 part; caches the answer per device.
+// Checks that the current device is an sm_100 part; caches the answer per device (thread-safe).
 mf_status require_sm100();
 int sm_count();
+
+// Thread-local "validate only" switch.  While it is set, every device entry point runs its complete argument / shape /
+// device validation and returns MF_OK just before its first enqueue.  The *_host entry points use it to validate the
+// whole chain of calls they are about to make BEFORE they allocate or copy anything ("on any error nothing has been
+// enqueued", include/mf.h).
+bool& validate_only();
+struct ValidateOnlyScope {
+    ValidateOnlyScope() { validate_only() = true; }
+    ~ValidateOnlyScope() { validate_only() = false; }
+};
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 

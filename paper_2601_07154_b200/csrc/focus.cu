@@ -529,10 +529,12 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
     __syncthreads();
     const int n_surv = s_count;
     if (n_surv > kMaxSurvivors) {
-        // more survivors than the list holds (huge sigma): fall back to this CTA's whole share of the tiles
-        for (int i = warp; i * kNormBlocks + part < n_tiles; i += 8)
+        // more survivors than the list holds (huge sigma): fall back to this CTA's whole share of the tiles, i.e. the
+        // SAME partition as the scan above (tile = i * kWarpsPerFrame + gw), so that a CTA that overflowed and one that
+        // did not still cover every surviving tile between them
+        for (int i = 0; i * kWarpsPerFrame + gw < n_tiles; ++i)
             exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
-                                                    i * kNormBlocks + part, tc, lane)));
+                                                    i * kWarpsPerFrame + gw, tc, lane)));
     } else {
         for (int i = warp; i < n_surv; i += 8)
             exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
@@ -577,27 +579,20 @@ __device__ __forceinline__ void st_stream(float4* p, float4 v) {
     asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
-// rows [ya, yb) of this thread's 4 columns where the map is identically zero: M = 0, G = 0 * D (depth is still read)
+// rows [ya, yb) of this thread's 4 columns where the map is identically zero: M = 0 and G = 0 (reading G1: the guided depth
+// is 0 wherever the map is 0, whatever the depth holds there, so the depth is not read)
 template <bool HAS_DEPTH, bool HAS_G, bool LOWRES>
 __device__ __forceinline__ void stream_zero_rows(const float* __restrict__ depth, float* __restrict__ focus_map,
                                                  float* __restrict__ guided, size_t img, int width, int ya, int yb) {
     constexpr int U = 8;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int y = ya; y < yb; y += U) {
-        float4 d[U];
-        if (HAS_G && !LOWRES) {
-#pragma unroll
-            for (int r = 0; r < U; ++r)
-                if (y + r < yb) d[r] = ld_stream(reinterpret_cast<const float4*>(depth + img + static_cast<size_t>(y + r) * width));
-        }
 #pragma unroll
         for (int r = 0; r < U; ++r) {
             if (y + r < yb) {
                 const size_t o = img + static_cast<size_t>(y + r) * width;
                 st_stream(reinterpret_cast<float4*>(focus_map + o), zero);
-                if (HAS_G)          // LOWRES: the interpolated depth is finite wherever its samples are, 0 * D = 0 is not read back
-                    st_stream(reinterpret_cast<float4*>(guided + o),
-                              LOWRES ? zero : make_float4(0.f * d[r].x, 0.f * d[r].y, 0.f * d[r].z, 0.f * d[r].w));
+                if (HAS_G) st_stream(reinterpret_cast<float4*>(guided + o), zero);
             }
         }
     }
@@ -757,7 +752,8 @@ render_kernel(const float* __restrict__ ex, const float* __restrict__ eyt, const
                     st_stream(reinterpret_cast<float4*>(focus_map + o), m);
                     if (HAS_G)
                         st_stream(reinterpret_cast<float4*>(guided + o),
-                                  make_float4(m.x * d[r].x, m.y * d[r].y, m.z * d[r].z, m.w * d[r].w));
+                                  make_float4(m.x != 0.f ? m.x * d[r].x : 0.f, m.y != 0.f ? m.y * d[r].y : 0.f,
+                                              m.z != 0.f ? m.z * d[r].z : 0.f, m.w != 0.f ? m.w * d[r].w : 0.f));     // reading G1
                 }
             }
         }
@@ -838,8 +834,9 @@ static mf_status motion_focus_impl(const double* global_w2c, mf_intrinsics K, in
 
     const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
     const size_t smem = sizeof(float) * (npad * static_cast<size_t>(tc + tr) + kMaxPoints + 8 * kTile * kMaxPoints);
+    if (focus_map && smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
+    if (validate_only()) return MF_OK;
     if (focus_map) {
-        if (smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
         if (smem > 48 * 1024)
             MF_CUDA_OK(cudaFuncSetAttribute(norm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     }

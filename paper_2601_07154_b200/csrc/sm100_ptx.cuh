@@ -39,8 +39,19 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
+// Bounded wait: try_wait already suspends the thread for a hardware time slice per attempt; after kSpinFast failed
+// attempts the thread backs off with nanosleep, and after kSpinLimit more (seconds, against waits that last
+// microseconds when the protocol is right) it traps, so a pipeline-protocol bug surfaces as a CUDA error
+// (MF_ERR_CUDA at the next runtime call) instead of hanging the GPU.
+constexpr uint32_t kSpinFast = 1u << 14, kSpinLimit = 1u << 25;
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
+        if (++spins > kSpinFast) {
+            __nanosleep(128);
+            if (spins > kSpinFast + kSpinLimit) __trap();
+        }
     }
 }
 

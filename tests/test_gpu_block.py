@@ -124,3 +124,33 @@ def test_block_forward_vs_oracle(api, windows, w, p, heads, d_hidden, head_dim, 
     x2 = x.clone()
     api.block_forward(x2, wts, windows, w, p, heads, mode, out=x2)
     assert torch.equal(x2, y)
+
+
+@pytest.mark.parametrize("mode_name", ["global", "frame"])
+@pytest.mark.parametrize("windows,w,p,heads,d_hidden,head_dim", [(2, 2, 100, 4, 1024, 64), (1, 2, 150, 4, 1024, 128)])
+def test_block_forward_vs_unrounded_oracle(api, windows, w, p, heads, d_hidden, head_dim, mode_name):
+    # The MATHEMATICAL block (oracle.block.block_forward with store = identity: no rounding anywhere, fp64) against the
+    # kernels, so that the check does not depend on the oracle imitating where the kernels store bf16 (reading E5).
+    # Tolerance: the path stores seven bf16 tensors (LN1 out, q|k|v, attention out, h, LN2 out, GELU out, y),
+    # each a relative perturbation of at most u = 2^-9 per element; the synthetic layers are norm-preserving on average
+    # (weights ~ N(0, 1/fan_in)), softmax averaging and LN (unit-variance rows) do not amplify, GELU is 1.13-Lipschitz, so
+    # to first order  ||y - y_exact|| / ||y_exact|| <= 7 u = 1.37e-2  (expected ~ sqrt(7) u / sqrt(3) = 3e-3),
+    # and per element  |d| <= u |ref| (y's own rounding) + 16 u rms(ref) (six propagated roundings, > 6 sigma).
+    from oracle import attention as oa
+    mode = oa.GLOBAL if mode_name == "global" else oa.FRAME
+    d = heads * head_dim
+    s_len = w * p
+    x = synth.tokens(windows * s_len, d, seed=70 + windows + heads, device="cuda")
+    wts = synth.block_weights(d, d_hidden, seed=110 + heads, device="cuda")
+    y = api.block_forward(x, wts, windows, w, p, heads, mode)
+    torch.cuda.synchronize()
+    w64 = {k: _to64(v) for k, v in wts.items()}
+    u = 2.0 ** -9
+    for n in range(windows):
+        ref = ob.block_forward(_to64(x[n * s_len:(n + 1) * s_len]), w64, w, p, heads, mode, oa.window_attention,
+                               store=lambda a: a)
+        dlt = _to64(y[n * s_len:(n + 1) * s_len]) - ref
+        rel = np.linalg.norm(dlt) / np.linalg.norm(ref)
+        rms = np.sqrt(np.mean(ref * ref))
+        assert rel <= 7 * u, rel
+        assert (np.abs(dlt) <= u * np.abs(ref) + 16 * u * rms).all(), float((np.abs(dlt) - u * np.abs(ref)).max() / (u * rms))

@@ -230,6 +230,62 @@ def test_focus_with_upsampled_depth(api, cfg_idx, n_frames, rb, re_, lo):
     assert worst <= 1.0, worst
 
 
+@pytest.mark.parametrize("sigma", [3000.0, 60000.0, 1.0e6])
+def test_focus_4k_huge_sigma_vs_oracle(api, sigma):
+    # 3840x2160 has 8160 bound tiles; with a very flat map most of them survive the branch-and-bound of the MAX normaliser
+    # and the per-CTA survivor list (256 entries) overflows: the fallback must still evaluate every surviving tile
+    cfg = synth.CONFIGS[4]
+    poses = synth.trajectory(cfg, synth.seed_for(4, 1), 20)
+    worst, fm, _ = _focus_case(api, poses, (cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"]), cfg["width"], cfg["height"],
+                               None, render_begin=19, render_end=20, sigma=sigma)
+    assert worst <= 1.0, worst
+    assert abs(float(fm.max()) - 1.0) <= 1e-5
+
+
+def test_focus_4k_sigma_sweep_max_is_one(api):
+    # The survivor count grows with sigma from a handful to all 8160 tiles; somewhere in between only SOME of the 8 CTAs
+    # of a frame overflow their list.  Whatever the split, the MAX-normalised map must peak at exactly 1 (within the bar):
+    # a surviving tile that nobody evaluates shows up as max(M) > 1.
+    cfg = synth.CONFIGS[4]
+    poses = torch.from_numpy(synth.trajectory(cfg, synth.seed_for(4, 1), 24)).cuda()
+    k = (cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"])
+    for mag, sigmas in ((1, np.geomspace(2.0e4, 4.0e5, 40)), (0, np.geomspace(2.0e5, 1.0e7, 24))):
+        for sigma in sigmas:
+            prm = api.focus_params(n_points=15, sigma=float(sigma), mag=mag)
+            out = api.motion_focus(poses, *k, cfg["width"], cfg["height"], prm, render_begin=20, render_end=24, want_guided=False)
+            peak = out["focus_map"].amax(dim=(1, 2)).cpu().numpy()
+            assert np.all(np.abs(peak - 1.0) <= 1e-5), (mag, sigma, peak)
+
+
+def test_guided_depth_is_zero_where_map_is_zero(api):
+    # reading G1 (include/mf.h): G = 0 exactly wherever M = 0, whatever the depth holds there; inside the map's support a
+    # non-finite depth sample propagates.  Same semantics for the full-resolution and the interpolated-depth call.
+    cfg = synth.CONFIGS[2]
+    w, h = cfg["width"], cfg["height"]
+    k = (cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"])
+    poses = torch.from_numpy(synth.trajectory(cfg, synth.seed_for(2, 1), 24)).cuda()
+    prm = api.focus_params(n_points=15, sigma=20.0)
+    depth = synth.depth(4, h, w, 5, device="cuda")
+    base = api.motion_focus(poses, *k, w, h, prm, depth=depth, render_begin=20, render_end=24)
+    m = base["focus_map"]
+    assert (m == 0).float().mean() > 0.3 and (m > 0).any()
+    bad = depth.clone()
+    bad[:, ::7, ::5] = float("nan")
+    bad[:, 3::11, 2::13] = float("inf")
+    out = api.motion_focus(poses, *k, w, h, prm, depth=bad, render_begin=20, render_end=24)
+    assert torch.equal(out["focus_map"], m)
+    g = out["guided_depth"]
+    assert (g[m == 0] == 0).all()
+    live = m > 0
+    assert torch.equal(torch.isfinite(g[live]), torch.isfinite(bad[live]))
+    assert torch.equal(g[live & torch.isfinite(bad)], base["guided_depth"][live & torch.isfinite(bad)])
+    lo = synth.depth(4, 294, 518, 6, device="cuda")
+    lo[:, ::9, ::4] = float("nan")
+    up = api.motion_focus_upsampled(poses, *k, w, h, lo, prm, render_begin=20, render_end=24)
+    assert torch.equal(up["focus_map"], m) and (up["guided_depth"][m == 0] == 0).all()
+    assert torch.isnan(up["guided_depth"][live]).any()
+
+
 def test_focus_degenerate_inputs(api):
     k = (200.0, 200.0, 112.0, 112.0)
     ident = np.tile(np.eye(4), (6, 1, 1))
