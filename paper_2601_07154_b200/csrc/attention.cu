@@ -27,6 +27,7 @@
 #include <cuda_bf16.h>
 
 #include <atomic>
+#include <mutex>
 
 namespace mf {
 
@@ -55,6 +56,7 @@ struct AttnSmem {
     alignas(8) uint64_t q_full;
     uint64_t k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages];
     uint64_t s_full[kQTiles], s_free[kQTiles], p_full[2][kQTiles], pv_done[2][kQTiles];   // [half][tile]
+    uint64_t roles_done;   // arrivals: the 11 role warps when they leave their loops (watchdog, sm100_ptx.cuh)
     uint32_t tmem_base;
     uint32_t zero;     // always 0 (see the softmax loop)
 };
@@ -116,6 +118,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             }
         }
         sm.zero = 0;
+        ptx::mbar_init(&sm.roles_done, 11);
         ptx::fence_barrier_init();
     }
     {   // ones tile: logical (key r, column 0) = 1.0 under the 128-byte swizzle, everything else 0
@@ -187,7 +190,13 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     ptx::mma_commit(&sm.v_empty[st]);
                 }
             }
+        } else if (lane == 0) {
+            ptx::watchdog(&sm.roles_done);            // warp 11: traps if the 11 role warps do not finish within seconds
         }
+#ifdef MF_AUX_SYNCWARP
+        __syncwarp();
+#endif
+        if (warp <= 10 && lane == 0) ptx::mbar_arrive(&sm.roles_done);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
         // ===================== softmax warpgroups =====================
@@ -217,6 +226,10 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 #pragma unroll
                         for (int i = 0; i < 32; ++i)
                             if (32 * c + i >= valid) s[c][i] = 0xff800000u;      // -inf
+                    // (MUFU lanes turn -inf into an exact 0; the polynomial lanes clamp to 2^-125.  Either way the key
+                    // adds nothing to O: TMA zero-fills the V rows past the sequence end (FLOAT_OOB_FILL_NONE), and it
+                    // adds at most 2^-125 per key to the row sum l >= 1.  Zeroing those words exactly was measured: a
+                    // uniform branch with 96 selects on every tail tile costs 6 % in FRAME mode, for no change in O.)
                 }
                 float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
@@ -324,6 +337,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 }
             }
         }
+        if (lane == 0) ptx::mbar_arrive(&sm.roles_done);
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -333,7 +347,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 }  // namespace mf
 
 // ------------------------------------------------------------------------------------------------
-// Host side: tensor maps + launch
+// Host side: tensor maps (cached) + launch
 // ------------------------------------------------------------------------------------------------
 namespace mf {
 
@@ -351,6 +365,39 @@ static mf_status make_map(CUtensorMap* map, const void* base, int sequences, int
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(MF_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", static_cast<int>(r));
+    return MF_OK;
+}
+
+// Per-process tensor-map cache.  A map depends only on (base pointer, sequences, seq_len, heads): the
+// layer stack of a window calls with the same q/k/v 24 times, a stream with the same static buffers for every window.
+// Small direct-mapped table under a mutex; an entry is the encoded 128-byte map, so a hit is one compare and one copy.
+struct MapKey {
+    const void* base;
+    int sequences, seq_len, heads;
+    bool operator==(const MapKey& o) const { return base == o.base && sequences == o.sequences && seq_len == o.seq_len && heads == o.heads; }
+};
+static mf_status cached_map(CUtensorMap* out, const void* base, int sequences, int seq_len, int heads) {
+    constexpr int kSlots = 64;
+    static std::mutex mu;
+    static MapKey keys[kSlots];
+    static CUtensorMap maps[kSlots];
+    static bool used[kSlots];
+    const MapKey key{base, sequences, seq_len, heads};
+    uint64_t h = reinterpret_cast<uintptr_t>(base) >> 8;
+    h = (h ^ (h >> 17) ^ (static_cast<uint64_t>(seq_len) * 0x9E3779B97F4A7C15ull) ^ (static_cast<uint64_t>(sequences) << 7) ^ heads) % kSlots;
+    {
+        std::lock_guard<std::mutex> g(mu);
+        if (used[h] && keys[h] == key) {
+            *out = maps[h];
+            return MF_OK;
+        }
+    }
+    mf_status st = make_map(out, base, sequences, seq_len, heads);
+    if (st != MF_OK) return st;
+    std::lock_guard<std::mutex> g(mu);
+    keys[h] = key;
+    maps[h] = *out;
+    used[h] = true;
     return MF_OK;
 }
 
@@ -383,6 +430,9 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if (static_cast<long long>((seq_len + 255) / 256) * heads * sequences > 0x7fffffffLL)
         return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     if (validate_only()) return MF_OK;
+    if (static_cast<long long>((seq_len + 255) / 256) * heads * sequences > 0x7fffffffLL)
+        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
+    if (validate_only()) return MF_OK;
 
     AttnParams prm;
     prm.seq_len = seq_len;
@@ -397,11 +447,10 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
         return launch_attention_d128(q, k, v, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
 
     CUtensorMap mq, mk, mv;
-    if ((st = make_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
-    if ((st = make_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
-    if ((st = make_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = cached_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = cached_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = cached_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
-    if (grid > 0x7fffffffLL) return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
     {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
         static std::atomic<bool> attr_set[64];

@@ -49,6 +49,7 @@ struct Smem {
     alignas(8) uint64_t q_full;
     uint64_t k_full[kStages], k_empty[kStages], v_full[kStages], v_empty[kStages];
     uint64_t s_full[kQTiles], s_free[kQTiles], p_full[kQTiles], pv_done[kQTiles];
+    uint64_t roles_done;   // arrivals: the 11 role warps when they leave their loops (watchdog, sm100_ptx.cuh)
     uint32_t tmem_base;
 };
 
@@ -105,6 +106,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
             ptx::mbar_init(&sm.p_full[t], 4);
             ptx::mbar_init(&sm.pv_done[t], 1);
         }
+        ptx::mbar_init(&sm.roles_done, 11);
         ptx::fence_barrier_init();
     }
     {   // ones atoms: logical (key r, column 0) = 1.0 under the 128-byte swizzle, everything else 0
@@ -176,7 +178,10 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                     ptx::mma_commit(&sm.v_empty[st]);
                 }
             }
+        } else if (lane == 0) {
+            ptx::watchdog(&sm.roles_done);            // warp 11: traps if the 11 role warps do not finish within seconds
         }
+        if (warp <= 10 && lane == 0) ptx::mbar_arrive(&sm.roles_done);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
         // ===================== softmax warpgroups =====================
@@ -301,6 +306,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                         static_cast<size_t>(frame) * prm.seq_len + row] = (m_used + log2f(l)) * 0.6931471805599453f;
             }
         }
+        if (lane == 0) ptx::mbar_arrive(&sm.roles_done);
     }
     ptx::tc_fence_before();
     __syncthreads();
