@@ -36,6 +36,7 @@ def parse_args():
     ap.add_argument("--no-stream", action="store_true", help="skip the per-window streaming latency measurement (SURVEY 8(f) NEXT-2)")
     ap.add_argument("--no-d128", action="store_true", help="skip the head_dim 128 attention measurement (SURVEY 8(f) NEXT-3)")
     ap.add_argument("--no-block", action="store_true", help="skip the whole-transformer-block measurement (SURVEY 8(f) NEXT-1)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE.json configs (SURVEY 8(d))")
     return ap.parse_args()
 
 
@@ -49,13 +50,22 @@ def measured_peaks():
     return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, source="fallback")
 
 
-# DRAM traffic per GLOBAL attention launch from the committed ncu captures (profiles/r1_ncu_full_v3.md), keyed by
-# (config index, windows per launch).  Other launch shapes have no capture: null.
-NCU_TRAFFIC_BYTES = {(3, 1): 152.94e6 + 34.52e6, (3, 4): 612.33e6 + 187.98e6}
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_ncu_attn_traffic.csv")
 
 
 def ncu_traffic(cfg_idx, windows_per_launch):
-    return NCU_TRAFFIC_BYTES.get((cfg_idx, windows_per_launch))
+    """DRAM bytes per GLOBAL attention launch (dram__bytes_read.sum + dram__bytes_write.sum) of the committed `ncu --set full`
+    capture of this launch shape, read from profiles/r2_ncu_attn_traffic.csv (text; written from the .ncu-rep, see the .md
+    beside it).  It is NOT measured in this run (ncu cannot run inside the timed bench); no capture of the shape -> None."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for ln in f:
+                parts = [x.strip() for x in ln.split(",")]
+                if len(parts) >= 4 and parts[0].isdigit() and (int(parts[0]), int(parts[1])) == (cfg_idx, windows_per_launch):
+                    return float(parts[2]) + float(parts[3])
+    except OSError:
+        pass
+    return None
 
 
 class ClockSampler:
@@ -135,6 +145,25 @@ class Workload:
         self.flops_step = self.Nw * (self.n_global * self.flops_global + self.n_frame * self.flops_frame)
         self.focus_bytes_step = 12.0 * self.N * self.width * self.height
 
+    @staticmethod
+    def launches_per_step(cfg_idx, args, api):
+        """Kernels of ours launched by one step_device() pass: one per (launch batch, layer), the pose chain, and 3 per focus call
+        (tables, norm, render)."""
+        w = Workload.__new__(Workload)
+        Workload.__init__(w, cfg_idx, args, None)
+        return ((w.Nw + w.B - 1) // w.B) * w.layers + 1 + 3 * ((w.N + w.chunk - 1) // w.chunk)
+
+    @staticmethod
+    def flops_per_step(cfg_idx, args, api):
+        w = Workload.__new__(Workload)
+        Workload.__init__(w, cfg_idx, args, None)
+        return w.flops_step
+
+    def release_host(self):
+        for name in ("hq", "hk", "hv", "ho", "hlocal", "hdepth", "hout", "hstreams"):
+            if hasattr(self, name):
+                delattr(self, name)
+
     # ---- device-resident inputs ----
     def setup_device(self):
         torch, synth = self.torch, self.synth
@@ -142,7 +171,7 @@ class Workload:
         self.q, self.k, self.v = synth.qkv(self.Nw, self.S, self.H, self.D, synth.seed_for(self.cfg_idx, 0), device=dev)
         self.o = [torch.empty((self.B, self.S, self.H, self.D), device=dev, dtype=torch.bfloat16) for _ in range(2)]
         traj = synth.trajectory(self.cfg, synth.seed_for(self.cfg_idx, 1), self.N)
-        self.local_np = synth.local_windows(traj, self.W, api.window_starts(self.N, self.W, self.stride), seed=synth.seed_for(self.cfg_idx, 2),
+        self.local_np = synth.local_windows(traj, self.W, self.api.window_starts(self.N, self.W, self.stride), seed=synth.seed_for(self.cfg_idx, 2),
                                             perturb_rot=1e-3, perturb_t=1e-3)
         self.local = torch.from_numpy(self.local_np).to(dev)
         self.depth = synth.depth(self.N, self.height, self.width, synth.seed_for(self.cfg_idx, 3), device=dev)
@@ -186,7 +215,7 @@ class Workload:
             if ev_focus is not None:
                 e1.record()
                 ev_focus.append((e0, e1, f1 - f0))
-            launches += 4
+            launches += 3
         self.launches = launches
         return poses
 
@@ -575,6 +604,112 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def timed_steps(wl, steps, warmup, barrier, reduce_max, gpu_index):
+    """W untimed + K timed passes of the whole hot path, bracketed by a barrier and CUDA events; clocks sampled meanwhile."""
+    import torch
+    for _ in range(warmup):
+        wl.step_device()
+    sampler = ClockSampler(gpu_index)
+    ev_g, ev_f = [], []
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        wl.step_device(ev_g, ev_f)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = reduce_max(e0.elapsed_time(e1))
+    g_ms = sum(a.elapsed_time(b) for a, b, _ in ev_g)
+    g_windows = sum(n for _, _, n in ev_g)
+    f_ms = sum(a.elapsed_time(b) for a, b, _ in ev_f)
+    f_frames = sum(n for _, _, n in ev_f)
+    focus_gbs = 12.0 * f_frames * wl.width * wl.height / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
+    # Bytes the call has to move: M and G are written everywhere (8 B/pixel), D is read only where the map is non-zero
+    # (reading G1: G = 0 wherever M = 0).  The render pass decides per warp (128 columns x one 32-row strip), so the share
+    # of such blocks of the first chunk's maps that hold a non-zero pixel estimates the share of pixels whose depth is read.
+    n = min(wl.chunk, wl.N)
+    live = torch.nn.functional.max_pool2d((wl.fmap[:n] != 0).to(torch.float16).unsqueeze(1), kernel_size=(32, 128), ceil_mode=True)
+    live_share = float(live.float().mean())
+    return dict(ms_total=ms_total, ms_step=ms_total / steps, clocks=clocks, g_ms=g_ms, g_windows=g_windows, g_launches=len(ev_g),
+                f_ms=f_ms, f_frames=f_frames,
+                tflops=wl.flops_global * g_windows / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0,
+                focus_gbs=focus_gbs, focus_live_share=live_share, focus_moved_gbs=focus_gbs * (8.0 + 4.0 * live_share) / 12.0)
+
+
+def measure_windows_per_launch(wl, torch, api, peak_sustained, batches=(1, 2, 4, 8)):
+    """the GLOBAL launch of this workload with 1, 2, 4 and 8 windows per launch, ~0.4 s of back-to-back launches each."""
+    out = {}
+    for b in batches:
+        if b > wl.Nw:
+            continue
+        q, k, v = wl.q[:b], wl.k[:b], wl.v[:b]
+        o = torch.empty_like(q)
+        for _ in range(2):
+            api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o); e1.record()
+        torch.cuda.synchronize()
+        n = max(3, int(400.0 / max(e0.elapsed_time(e1), 1e-3)))
+        e0.record()
+        for _ in range(n):
+            api.window_attention(q, k, v, wl.W, wl.P, api.ATTN_GLOBAL, out=o)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n
+        tf = wl.flops_global * b / (ms * 1e-3) / 1e12
+        out[str(b)] = {"ms_per_launch": ms, "tflops": tf, "frac_of_sustained_peak": tf / peak_sustained}
+    return out
+
+
+def oracle_full_small(cfg_idx, dims):
+    """SURVEY 8(d) procedure 4 for the two small configs: the oracle evaluated IN FULL, not on sampled rows -- the whole clip for
+    the tiny config; one whole window (every row of one FRAME and one GLOBAL layer) for the suburban config, the clip's other
+    windows and layers being repeats of the same work (stated as such).  Returns a cpu_baseline block."""
+    import numpy as np
+    from oracle import attention as oa
+    from oracle import chain as oc
+    from oracle import points as op
+    from oracle import render as orr
+    from oracle import windows as ow
+    from paper_2601_07154_b200 import synth
+    cfg = synth.CONFIGS[cfg_idx]
+    W, P, H, D, S, Nw, N, layers = (dims[k] for k in ("W", "P", "H", "D", "S", "Nw", "N", "layers"))
+    q, k, v = (t.float().numpy().astype(np.float64) for t in synth.qkv(1, S, H, D, synth.seed_for(cfg_idx, 0)))
+    t0 = time.perf_counter()
+    oa.window_attention(q, k, v, W, P, oa.GLOBAL)
+    t_global = time.perf_counter() - t0
+    t_frame = 0.0
+    if layers > 1:
+        t0 = time.perf_counter()
+        oa.window_attention(q, k, v, W, P, oa.FRAME)
+        t_frame = time.perf_counter() - t0
+    traj = synth.trajectory(cfg, synth.seed_for(cfg_idx, 1), N)
+    loc = synth.local_windows(traj, W, ow.window_starts(N, W, cfg["stride"]), seed=synth.seed_for(cfg_idx, 2), perturb_rot=1e-3, perturb_t=1e-3)
+    t0 = time.perf_counter()
+    poses = oc.chain_poses(loc.tolist(), W, cfg["stride"], N)
+    frames = op.motion_points(poses, cfg["fx"], cfg["fy"], cfg["cx"], cfg["cy"], cfg["width"], cfg["height"], 15, cfg["sigma"])
+    t_pose = time.perf_counter() - t0
+    n_render = N if cfg_idx == 0 else 2
+    depth = synth.depth(n_render, cfg["height"], cfg["width"], synth.seed_for(cfg_idx, 3)).numpy()
+    t0 = time.perf_counter()
+    for f in range(n_render):
+        orr.focus_map(frames[N - 1 - f]["points"], cfg["width"], cfg["height"], orr.NORM_MAX, depth[f])
+    t_render = (time.perf_counter() - t0) / n_render
+    n_global = layers // 2 if layers > 1 else 1
+    n_frame = layers - n_global
+    total = Nw * (n_global * t_global + n_frame * t_frame) + t_pose + N * t_render
+    whole = cfg_idx == 0
+    return {"value": N / total, "unit": "frames/s", "kind": "oracle", "cores": len(os.sched_getaffinity(0)),
+            "sample": ("whole clip evaluated in full" if whole else
+                       f"one whole window evaluated in full (all {S} rows x {H} heads, one GLOBAL layer {t_global:.2f}s + one FRAME layer "
+                       f"{t_frame:.2f}s), pose chain + motion points of the whole clip ({t_pose:.2f}s), Eq.7 render of {n_render} frames "
+                       f"({t_render:.2f}s each); the other {Nw - 1} windows, {layers - 2} layers and {N - n_render} frames repeat this work: "
+                       f"whole-clip seconds = {total:.0f}"),
+            "seconds_measured": t_global + t_frame + t_pose + t_render * n_render}
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -597,42 +732,28 @@ def main():
     def reduce_max(x):
         return replicas.max_over_ranks(x, dev)
 
-    for _ in range(args.warmup):
-        wl.step_device()
-    sampler = ClockSampler(local_rank)
-    ev_g, ev_f = [], []
-    barrier()
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        wl.step_device(ev_g, ev_f)
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    ms_total = reduce_max(e0.elapsed_time(e1))
-    ms_step = ms_total / args.steps
+    res = timed_steps(wl, args.steps, args.warmup, barrier, reduce_max, local_rank)
+    ms_total, ms_step, clocks = res["ms_total"], res["ms_step"], res["clocks"]
     value = replicas.whole_job_value(wl.N, ms_step, world)
-
-    g_ms = sum(a.elapsed_time(b) for a, b, _ in ev_g)
-    g_windows = sum(n for _, _, n in ev_g)
-    g_launch_ms = g_ms / max(len(ev_g), 1)
-    tflops = wl.flops_global * g_windows / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
-    f_ms = sum(a.elapsed_time(b) for a, b, _ in ev_f)
-    f_frames = sum(n for _, _, n in ev_f)
-    focus_gbs = 12.0 * f_frames * wl.width * wl.height / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
+    tflops, focus_gbs = res["tflops"], res["focus_gbs"]
+    traffic = ncu_traffic(args.config, wl.B)
     roofline = {"bound": "tensor", "kernel": "window_attention_kernel (GLOBAL mode)", "achieved": tflops,
                 "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": tflops / peaks["tf_sustained"],
                 "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['source']}); kernel timed inside a long step",
                 "frac_of_burst": tflops / peaks["tf_burst"], "frac_of_nominal_2250": tflops / 2250.0,
-                "flops_per_launch": wl.flops_global * wl.B, "ms_per_launch": g_launch_ms,
-                "share_of_step": g_ms / ms_total, "traffic": ncu_traffic(args.config, wl.B),
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this "
-                                  "launch shape (profiles/r1_ncu_full_v3.md); algorithmic Q,K,V,O bytes per launch = "
-                                  f"{8.0 * wl.S * wl.H * wl.D * wl.B:.0f}"}
-    focus = {"bound": "hbm", "kernel": "mf_motion_focus (points+tables+norm+render, 12 B/pixel algorithmic)",
+                "flops_per_launch": wl.flops_global * wl.B, "ms_per_launch": res["g_ms"] / max(res["g_launches"], 1),
+                "share_of_step": res["g_ms"] / ms_total, "traffic": traffic,
+                "traffic_source": "NOT measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of the committed `ncu --set full` "
+                                  "capture of this launch shape (profiles/r2_ncu_attn.md, r2_ncu_attn_traffic.csv); algorithmic Q,K,V,O "
+                                  f"bytes per launch = {8.0 * wl.S * wl.H * wl.D * wl.B:.0f}"}
+    focus = {"bound": "hbm", "kernel": "mf_motion_focus (points+tables+norm+render, 12 B/pixel algorithmic: read D, write M, write G)",
              "achieved": focus_gbs, "peak": peaks["hbm"], "unit": "GB/s", "frac": focus_gbs / peaks["hbm"],
-             "share_of_step": f_ms / ms_total}
+             "share_of_step": res["f_ms"] / ms_total,
+             "bytes_moved": {"gbs": res["focus_moved_gbs"], "frac": res["focus_moved_gbs"] / peaks["hbm"],
+                             "per_pixel": 8.0 + 4.0 * res["focus_live_share"], "depth_read_share": res["focus_live_share"]},
+             "note": "`achieved` counts SURVEY 8(d)'s algorithmic 12 B/pixel (read D, write M, write G).  Since round 2 the call does not "
+                     "read D where M is exactly zero (reading G1), so it MOVES fewer bytes: `bytes_moved` is the same time against "
+                     "8 B/pixel + 4 B/pixel x the estimated share of pixels whose depth is read (ncu: profiles/r2_ncu_focus.md)"}
 
     e2e = None
     if not args.no_e2e:
@@ -647,6 +768,7 @@ def main():
         sec = reduce_max((time.perf_counter() - t0) / n_e2e)
         e2e = {"value": world * wl.N / sec, "unit": "frames/s", "h2d_bytes_per_step": int(wl.h2d), "d2h_bytes_per_step": int(wl.d2h),
                "steps": n_e2e, "note": "mf_window_attention_host + mf_chain_and_focus_host on pinned host buffers, called from 4 host threads on 4 streams"}
+        wl.release_host()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -671,14 +793,56 @@ def main():
     if rank == 0 and not args.no_stream and wl.Nw >= 8 and wl.layers > 1:
         streaming = measure_streaming(wl, torch, api)
 
+    wpl = None
+    if rank == 0 and world == 1 and wl.Nw >= 8 and wl.layers > 1:
+        wpl = measure_windows_per_launch(wl, torch, api, peaks["tf_sustained"])
+
+    # every BASELINE.json config in the driver-run line.  After the headline step, the other four configs run
+    # 1 warm-up + 2 timed passes each (same step, same launch configuration), single GPU only.
+    per_config = None
+    launches_extra = 0
+    if rank == 0 and world == 1 and args.config == 3 and not args.no_per_config and not args.max_windows:
+        from paper_2601_07154_b200 import synth
+        per_config = {synth.CONFIGS[3]["name"]: {"frames_per_s": value, "ms_per_step": ms_step, "global_tflops": tflops,
+                                                 "frac_sustained": tflops / peaks["tf_sustained"], "focus_gbs": focus_gbs,
+                                                 "focus_frac": focus_gbs / peaks["hbm"], "focus_moved_gbs": res["focus_moved_gbs"],
+                                                 "focus_moved_frac": res["focus_moved_gbs"] / peaks["hbm"], "sm_mhz": clocks.get("sm_mhz"),
+                                                 "steps": args.steps, "window_size": wl.W}}
+        del wl
+        torch.cuda.empty_cache()
+        for ci in (0, 1, 2, 4):
+            w2 = Workload(ci, args, dev)
+            w2.setup_device()
+            steps2 = 20 if ci == 0 else 2
+            r2 = timed_steps(w2, steps2, 3 if ci < 2 else 1, barrier, reduce_max, local_rank)
+            entry = {"frames_per_s": w2.N / (r2["ms_step"] * 1e-3), "ms_per_step": r2["ms_step"], "global_tflops": r2["tflops"],
+                     "frac_sustained": r2["tflops"] / peaks["tf_sustained"], "focus_gbs": r2["focus_gbs"],
+                     "focus_frac": r2["focus_gbs"] / peaks["hbm"], "focus_moved_gbs": r2["focus_moved_gbs"],
+                     "focus_moved_frac": r2["focus_moved_gbs"] / peaks["hbm"], "sm_mhz": r2["clocks"].get("sm_mhz"),
+                     "reasons": r2["clocks"].get("reasons"), "steps": steps2, "window_size": w2.W,
+                     "workload": config_block(ci, dims_of(ci, args, api.num_windows), args)["workload"]}
+            if ci == 0:
+                entry["windows_148"] = measure_one_wave(w2, torch, api, peaks["tf_sustained"])
+            if ci in (0, 1) and not args.no_cpu_baseline:
+                entry["cpu_baseline"] = oracle_full_small(ci, dims_of(ci, args, api.num_windows))
+            launches_extra += w2.launches * steps2
+            per_config[synth.CONFIGS[ci]["name"]] = entry
+            del w2
+            torch.cuda.empty_cache()
+        wl = None
+
     if rank == 0:
         dims = dims_of(args.config, args, api.num_windows)
+        step_launches = Workload.launches_per_step(args.config, args, api)
         line = {"metric": "frames/sec at W=32 (window attention stack + pose chain + motion focus)", "value": value,
                 "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": config_block(args.config, dims, args, {"parallelism": f"replicas x{world} (one clip per GPU)"}),
-                "roofline": roofline, "focus_roofline": focus, "attention_tflops_all_layers": wl.flops_step * args.steps / (ms_total * 1e-3) / 1e12,
-                "cpu_baseline": cpu, "e2e": e2e, "block": block, "head_dim_128": d128, "windows_148": one_wave, "streaming": streaming, "gpu_launches": wl.launches * args.steps, "clocks": clocks}
+                "config": config_block(args.config, dims, args), "parallelism": f"replicas x{world} (one clip per GPU)",
+                "roofline": roofline, "focus_roofline": focus,
+                "attention_tflops_all_layers": Workload.flops_per_step(args.config, args, api) * args.steps / (ms_total * 1e-3) / 1e12,
+                "cpu_baseline": cpu, "e2e": e2e, "block": block, "head_dim_128": d128, "windows_148": one_wave, "streaming": streaming,
+                "windows_per_launch_sweep": wpl, "per_config": per_config,
+                "gpu_launches": step_launches * args.steps, "gpu_launches_per_config_runs": launches_extra, "clocks": clocks}
         print(json.dumps(line))
     replicas.finish()
 

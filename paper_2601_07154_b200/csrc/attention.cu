@@ -193,9 +193,6 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
         } else if (lane == 0) {
             ptx::watchdog(&sm.roles_done);            // warp 11: traps if the 11 role warps do not finish within seconds
         }
-#ifdef MF_AUX_SYNCWARP
-        __syncwarp();
-#endif
         if (warp <= 10 && lane == 0) ptx::mbar_arrive(&sm.roles_done);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
