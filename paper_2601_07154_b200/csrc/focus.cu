@@ -396,7 +396,7 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
     float* mx = sm_f;                       // [npad][tc] largest Ex_j over the tile's columns (Ex_j is unimodal)
     float* my = sm_f + npad * tc;           // [npad][tr]
     float* centre = my + npad * tr;         // [kMaxPoints] map value at each centre's pixel
-    float* tile_buf = centre + kMaxPoints;  // [8 warps][kTile rows][kMaxPoints] staged row factors
+    float* tile_buf = centre + kMaxPoints;  // [8 warps][kTile rows][npad] staged row factors
     if (threadIdx.x < kMaxPoints) {
         s_pts[threadIdx.x] = threadIdx.x < n_valid ? pts[static_cast<size_t>(f) * kMaxPoints + threadIdx.x]
                                                    : make_float4(0.f, 0.f, 1.f, 0.f);
@@ -513,7 +513,7 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
     const float best = __uint_as_float(s_best);
     float exact = 0.f;
     // tile t belongs to warp (t mod 8*kNormBlocks) of the frame: neighbouring (surviving) tiles go to different warps
-    constexpr int kWarpsPerFrame = 8 * kNormBlocks;
+    const int kWarpsPerFrame = 8 * static_cast<int>(gridDim.x);
     const int gw = part * 8 + warp;
     const int n_tiles = tc * tr;
     for (int i = lane; i * kWarpsPerFrame + gw < n_tiles; i += 32) {
@@ -533,11 +533,11 @@ norm_kernel(const float4* __restrict__ pts, FrameMeta* __restrict__ meta, const 
         // SAME partition as the scan above (tile = i * kWarpsPerFrame + gw), so that a CTA that overflowed and one that
         // did not still cover every surviving tile between them
         for (int i = 0; i * kWarpsPerFrame + gw < n_tiles; ++i)
-            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
+            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * npad), npad, width, height,
                                                     i * kWarpsPerFrame + gw, tc, lane)));
     } else {
         for (int i = warp; i < n_surv; i += 8)
-            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * kMaxPoints), npad, width, height,
+            exact = fmaxf(exact, warp_max(eval_tile(exf, eyf, tile_buf + warp * (kTile * npad), npad, width, height,
                                                     s_list[i], tc, lane)));
     }
     // only exactly evaluated pixels may set Z (the bound above is 0.9999 x an approximately summed value); the tile
@@ -833,7 +833,10 @@ static mf_status motion_focus_impl(const double* global_w2c, mf_intrinsics K, in
     pp.width = width; pp.height = height;
 
     const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
-    const size_t smem = sizeof(float) * (npad * static_cast<size_t>(tc + tr) + kMaxPoints + 8 * kTile * kMaxPoints);
+    const size_t smem = sizeof(float) * (npad * static_cast<size_t>(tc + tr) + kMaxPoints + 8 * kTile * npad);
+    // CTAs per frame in norm_kernel: kNormBlocks when the call is short, fewer when it holds so many frames that 8 per frame
+    // would need several waves of these latency-bound CTAs (8 x 256 threads fit one SM)
+    const int norm_blocks = std::max(1, std::min(kNormBlocks, (8 * sm_count() + count - 1) / count));
     if (focus_map && smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
     if (validate_only()) return MF_OK;
     if (focus_map) {
@@ -861,7 +864,7 @@ static mf_status motion_focus_impl(const double* global_w2c, mf_intrinsics K, in
                                                       uv, fi, ex, eyt, npad, width, height);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
-        return launch_pdl(norm_kernel, dim3(kNormBlocks, n), dim3(256), smem, q, ws.pts + static_cast<size_t>(f0) * kMaxPoints,
+        return launch_pdl(norm_kernel, dim3(norm_blocks, n), dim3(256), smem, q, ws.pts + static_cast<size_t>(f0) * kMaxPoints,
                           ws.meta + f0, ex, eyt, ws.colmask + static_cast<size_t>(f0) * tc, ws.rowmask + static_cast<size_t>(f0) * tr,
                           npad, width, height, static_cast<int>(params->norm));
     };
