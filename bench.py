@@ -27,7 +27,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = campus, W=32)")
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = campus, W=32); 5..11 = the rows of the paper's Table 2 (synth.CONFIGS)")
     ap.add_argument("--windows-per-launch", type=int, default=4)
     ap.add_argument("--focus-chunk", type=int, default=300, help="frames per mf_motion_focus call")
     ap.add_argument("--max-windows", type=int, default=0, help="debug: truncate the clip to this many windows")

@@ -38,6 +38,19 @@ CONFIGS = [
          step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.15, sigma=20.0),
 ]
 
+# The other six rows of the paper's Table 2 as workloads 6..11, same recipe as workload 5.  Resolution 384 at 16:9 with
+# 14-px patches -> 27 x 15 = 405 tokens/frame; "DA3 Small" is taken as ViT-S widths (6 heads x 64, 12 blocks): like the ViT-B
+# widths of "DA3 Base" an ASSUMPTION, not stated in PAPER.md.  Batch size = window W, overlap W/2.
+def _table2(name, w, p, heads):
+    return dict(name=name, W=w, stride=w // 2, N=600, P=p, H=heads, D=64, layers=12,
+                width=1920, height=1080, fx=1400.0, fy=1400.0, cx=960.0, cy=540.0, fps=30,
+                step=0.047, step_sd=0.01, rot_sd=0.02, head_yaw_sd=0.15, sigma=20.0)
+
+
+CONFIGS += [_table2("table2-base-384-b60", 60, 405, 12), _table2("table2-base-384-b30", 30, 405, 12),
+            _table2("table2-small-504-b60", 60, 720, 6), _table2("table2-small-384-b60", 60, 405, 6),
+            _table2("table2-small-504-b30", 30, 720, 6), _table2("table2-small-384-b30", 30, 405, 6)]
+
 
 def seed_for(config_index, stream):
     return BASE_SEED + 1000 * config_index + stream
