@@ -36,23 +36,28 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    if not force and not _stale():
-        return OUT
+def build(force=False, verbose=False, out=None, extra_flags=(), build_dir=None):
+    """Compiles every source and links the library.  `out` / `extra_flags` / `build_dir` build a variant somewhere else
+    (tests/test_gpu_watchdog.py builds one with an injected pipeline bug); the default is the in-tree product library."""
+    variant = out is not None
+    out = out or OUT
+    if not variant and not force and not _stale():
+        return out
     nvcc = _nvcc()
     objs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    build_dir = build_dir or os.path.join(HERE, "build")
+    os.makedirs(build_dir, exist_ok=True)
     for src in SOURCES:
-        obj = os.path.join(HERE, "build", src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + PER_FILE.get(src, []) + os.environ.get("MF_NVCC_EXTRA", "").split() + [
+        obj = os.path.join(build_dir, src.replace(".cu", ".o"))
+        cmd = [nvcc] + NVCC_FLAGS + PER_FILE.get(src, []) + os.environ.get("MF_NVCC_EXTRA", "").split() + list(extra_flags) + [
             "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             print(" ".join(cmd))
         subprocess.run(cmd, check=True)
         objs.append(obj)
-    cmd = [nvcc, "-shared", "-o", OUT] + objs + ["-cudart", "static"]
+    cmd = [nvcc, "-shared", "-o", out] + objs + ["-cudart", "static"]
     subprocess.run(cmd, check=True)
-    return OUT
+    return out
 
 
 if __name__ == "__main__":

@@ -218,7 +218,11 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 ptx::tc_wait_ld();
                 ptx::tc_fence_before();
                 __syncwarp();
+#ifdef MF_TEST_PROTOCOL_BUG      // test builds only (tests/test_gpu_watchdog.py): CTA 0 never hands S back, so its pipeline stalls for good
+                if (lane == 0 && blockIdx.x != 0) ptx::mbar_arrive(&sm.s_free[tile]);
+#else
                 if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by S(j+1)
+#endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
 #pragma unroll
