@@ -47,6 +47,10 @@ constexpr float kRescaleThreshold = 8.0f;          // log2 units
 #define MF_POLY_PAIRS 4                // of every 16 score pairs, this many are exponentiated on the FMA pipe
 #endif
 constexpr int kPolyPairs = MF_POLY_PAIRS;
+#ifndef MF_PERSISTENT_BELOW_TILES
+#define MF_PERSISTENT_BELOW_TILES 64   // sequences of fewer KV tiles (S <= 8064) run on the persistent kernel (attention_clc.cu)
+#endif
+constexpr int kPersistentBelowTiles = MF_PERSISTENT_BELOW_TILES;
 
 struct AttnSmem {
     alignas(1024) uint8_t q[kQTiles][kTileBytes];
@@ -82,11 +86,9 @@ __device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, 
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
 }
 
-template <bool kTmaStore>
 __global__ void __launch_bounds__(kThreads, 1)
 window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
-                        const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_o,
-                        const AttnParams prm) {
+                        const __grid_constant__ CUtensorMap map_v, const AttnParams prm) {
     extern __shared__ uint8_t smem_raw[];
     AttnSmem& sm = *reinterpret_cast<AttnSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -103,7 +105,6 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
         ptx::prefetch_tensormap(&map_q);
         ptx::prefetch_tensormap(&map_k);
         ptx::prefetch_tensormap(&map_v);
-        if (kTmaStore) ptx::prefetch_tensormap(&map_o);
         const uint32_t live = tile1_live ? 2 : 1;          // MMA issuers that release every K/V stage
         ptx::mbar_init(&sm.q_full, 1);
         for (int s = 0; s < kStages; ++s) {
@@ -320,34 +321,12 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const float l = __uint_as_float(ptx::tmem_ld1(t_o + kD));           // row sum from the ones column
             ptx::tc_wait_ld();
             const float inv_l = 1.0f / l;
-            // Two ways out for the 128 x 64 bf16 tile.  A thread's own row is 128 contiguous bytes but the rows of a warp
-            // are heads*128 bytes apart, so direct stores are 32 wavefronts per instruction (~1 us per CTA).  Staged
-            // through shared memory (this tile's Q tile: every Q K^T MMA that read it completed before the last S was
-            // published) the tile leaves in ONE TMA store (cp.async.bulk.tensor, SWIZZLE_128B, rows past the sequence end
-            // clipped by the tensor map), but the CTA must then outlive the TMA's read of shared memory.  Measured: the TMA
-            // store wins where CTAs are short (FRAME mode +1 %, S = 1024 +2 %, P = 256 frames +6 %) and loses 0.45 % on the
-            // 300-us CTAs of the campus window -- even as a run-time branch its mere presence cost the long launch 0.6 %, so
-            // the two epilogues are two instantiations and the host picks per launch (TMA store below 64 KV tiles).
-            if (kTmaStore) {
-                uint4* stage = reinterpret_cast<uint4*>(sm.q[tile]) + row_in_tile * 8;     // 8 chunks of 16 bytes per row
-#pragma unroll
-                for (int c = 0; c < 2; ++c)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        uint4 w;
-                        w.x = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 0]) * inv_l, __uint_as_float(o[c][8 * i + 1]) * inv_l);
-                        w.y = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 2]) * inv_l, __uint_as_float(o[c][8 * i + 3]) * inv_l);
-                        w.z = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 4]) * inv_l, __uint_as_float(o[c][8 * i + 5]) * inv_l);
-                        w.w = ptx::pack_bf16(__uint_as_float(o[c][8 * i + 6]) * inv_l, __uint_as_float(o[c][8 * i + 7]) * inv_l);
-                        stage[(4 * c + i) ^ (row_in_tile & 7)] = w;
-                    }
-                ptx::fence_proxy_async();                         // generic-proxy writes -> visible to the TMA (async proxy)
-                asm volatile("bar.sync %0, 128;" :: "r"(1 + tile) : "memory");      // the tile's four softmax warps
-                if (row_in_tile == 0) {
-                    ptx::tma_store_4d(&map_o, sm.q[tile], 0, head, row0 + tile * kBM, seq);
-                    ptx::tma_store_commit_and_wait_read();        // shared memory must outlive the read; the CTA exits next
-                }
-            } else if (row < prm.seq_len) {
+            // Direct stores: a thread's own row is 128 contiguous bytes, but the rows of a warp are heads*128 bytes apart
+            // (32 wavefronts per instruction, ~1 us per CTA).  That is 0.3 % of the 300-us CTAs this kernel is used for; the
+            // short sequences, where it shows, go to the persistent kernel (attention_clc.cu), which stages the tile in
+            // shared memory and sends it with one TMA store.  (A TMA-store epilogue here was measured: -0.45 % on the campus
+            // window because the CTA has to outlive the TMA's read of shared memory, -0.6 % even as a branch never taken.)
+            if (row < prm.seq_len) {
                 const size_t tok = static_cast<size_t>(seq) * prm.seq_len + row;
                 uint4* dst = reinterpret_cast<uint4*>(prm.out + (tok * prm.heads + head) * kD);
 #pragma unroll
@@ -486,18 +465,18 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if ((st = cached_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
-    const bool tma_store = (seq_len + kBN - 1) / kBN < 64;       // short CTAs: TMA store epilogue (see the kernel's epilogue)
-    auto kernel = tma_store ? window_attention_kernel<true> : window_attention_kernel<false>;
-    {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device and instantiation
-        static std::atomic<bool> attr_set[2][64];
+    if ((seq_len + kBN - 1) / kBN < kPersistentBelowTiles)      // short items: persistent kernel (cluster launch control)
+        return launch_attention_clc(mq, mk, mv, mo, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
+    {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
+        static std::atomic<bool> attr_set[64];
         int dev = 0;
         MF_CUDA_OK(cudaGetDevice(&dev));
-        if (dev < 0 || dev >= 64 || !attr_set[tma_store][dev].load(std::memory_order_acquire)) {
-            MF_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            if (dev >= 0 && dev < 64) attr_set[tma_store][dev].store(true, std::memory_order_release);
+        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
+            MF_CUDA_OK(cudaFuncSetAttribute(window_attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
         }
     }
-    kernel<<<static_cast<unsigned>(grid), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(mq, mk, mv, mo, prm);
+    window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(mq, mk, mv, prm);
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
 }

@@ -41,6 +41,11 @@ __device__ __forceinline__ void exp2_poly2(uint32_t& a0, uint32_t& a1) {
     a1 = p1 + (t1 << 23);
 }
 
+// head_dim 64, short sequences: persistent kernel driven by cluster launch control (attention_clc.cu); the caller supplies the
+// tensor maps of q, k, v and out (box 64 x 1 x 128 x 1, SWIZZLE_128B)
+mf_status launch_attention_clc(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
+                               int sequences, int seq_len, int heads, const AttnParams& prm, cudaStream_t stream);
+
 // head_dim 128 variant (attention_d128.cu); same contract as the head_dim 64 launch inside mf_window_attention
 mf_status launch_attention_d128(const void* q, const void* k, const void* v, int sequences, int seq_len, int heads,
                                 const AttnParams& prm, cudaStream_t stream);

@@ -93,6 +93,9 @@ __device__ __forceinline__ void tma_store_4d(const CUtensorMap* m, const void* s
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
                  :: "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// wait until every committed store has READ its shared memory
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 // commit the store(s) and wait until shared memory has been READ (the source may then be reused or the CTA may exit; the
 // global writes complete on their own and are visible at kernel end like any other store)
 __device__ __forceinline__ void tma_store_commit_and_wait_read() {
