@@ -179,25 +179,20 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     if (use > 0) ptx::mbar_wait(&sm.q_empty[slot], (use - 1) & 1);
                     ptx::mbar_arrive_expect_tx(&sm.q_full[slot], kQTiles * kTileBytes);
                     ptx::tma_load_4d(sm.q[slot][0], &map_q, &sm.q_full[slot], 0, it.head, it.row0(), it.seq);
-                    // a dead second tile re-reads the first one (in bounds, never used); nobody works on it, so the producer
-                    // makes its two arrivals on the Q slot and its issuer's arrival on every K/V stage of the item
+                    // a dead second tile re-reads the first one (in bounds, never used); no output store will read its staging
+                    // buffer, so the producer makes that arrival on the Q slot itself
                     const bool dead1 = !it.tile1_live(prm);
                     ptx::tma_load_4d(sm.q[slot][1], &map_q, &sm.q_full[slot], 0, it.head, dead1 ? it.row0() : it.row0() + kBM, it.seq);
-                    if (dead1) {
-                        ptx::mbar_arrive(&sm.q_empty[slot]);
-                        ptx::mbar_arrive(&sm.q_empty[slot]);
-                    }
+                    if (dead1) ptx::mbar_arrive(&sm.q_empty[slot]);
                     for (int j = 0; j < n_kv; ++j, ++kv) {
                         const int st = kv % kStages;
                         const uint32_t ph = (kv / kStages) & 1;
                         ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
                         ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
                         ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, it.head, j * kBN, it.seq);
-                        if (dead1) ptx::mbar_arrive(&sm.k_empty[st]);
                         ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
                         ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
                         ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, it.head, j * kBN, it.seq);
-                        if (dead1) ptx::mbar_arrive(&sm.v_empty[st]);
                     }
                     it = fetch_item(sm, qi + 1);
                 }
@@ -227,7 +222,21 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     const int slot = qi & 1;
                     const bool live = t == 0 || it.tile1_live(prm);
                     if (!live) {
-                        kv += n_kv;                         // nothing to compute for this tile slot (the producer made our arrivals)
+                        // Nothing to compute for this tile slot, but it stays a link of the flow control: it releases the Q slot
+                        // and every K/V stage of the item only after it has seen them filled.  (Parity waits tell only
+                        // neighbouring phases apart: an issuer that skipped these waits would later take a stage's previous fill
+                        // for the one it is waiting for, and one that only watched, with the producer making its arrivals, could
+                        // be lapped by the producer.  Both were tried; both deadlock on long runs of such items.)
+                        ptx::mbar_wait(&sm.q_full[slot], (qi >> 1) & 1);
+                        ptx::mbar_arrive(&sm.q_empty[slot]);
+                        for (int j = 0; j < n_kv; ++j, ++kv) {
+                            const int st = kv % kStages;
+                            const uint32_t ph = (kv / kStages) & 1;
+                            ptx::mbar_wait(&sm.k_full[st], ph);
+                            ptx::mbar_arrive(&sm.k_empty[st]);
+                            ptx::mbar_wait(&sm.v_full[st], ph);
+                            ptx::mbar_arrive(&sm.v_empty[st]);
+                        }
                         have_s = false;
                         it = fetch_item(sm, qi + 1);
                         continue;
@@ -305,7 +314,11 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 ptx::tc_wait_ld();
                 ptx::tc_fence_before();
                 __syncwarp();
+#ifdef MF_TEST_PROTOCOL_BUG      // test builds only (tests/test_gpu_watchdog.py): CTA (0,0,0) never hands S back, so its pipeline stalls for good
+                if (lane == 0 && (blockIdx.x | blockIdx.y | blockIdx.z) != 0) ptx::mbar_arrive(&sm.s_free[tile]);
+#else
                 if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by the next S
+#endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
 #pragma unroll

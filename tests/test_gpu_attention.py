@@ -83,6 +83,36 @@ def test_ragged_shapes(api, windows, w, p, heads, mode):
     _check(api, windows, w, p, heads, mode, 1234 + windows * 7 + w * 13 + p, lse=True)
 
 
+@pytest.mark.parametrize("w,p,heads,qscale", [
+    (1, 8200, 2, 1.0),       # 65 KV tiles, last q block holds 8 rows (second Q tile dead), 8 keys in the tail tile
+    (3, 2900, 1, 1.0),       # S = 8700: ragged second tile (252 rows in the last q block), 124-key tail
+    (2, 4160, 2, 4.0),       # S = 8320 = 65 x 128 exactly, peaked
+    (1, 8321, 1, 1.0),       # one key into the 66th tile
+])
+def test_ragged_shapes_long_sequences(api, w, p, heads, qscale):
+    # Sequences of 64 KV tiles and more run on the one-item-per-CTA kernel (attention.cu), shorter ones on the persistent
+    # kernel (attention_clc.cu): the ragged cases above the switch, GLOBAL mode, oracle on sampled rows (reading A7)
+    s_len = w * p
+    rng = np.random.default_rng(s_len)
+    rows = np.unique(np.concatenate([np.arange(64), np.arange(s_len - 300, s_len), rng.integers(0, s_len, 128)]))
+    _check(api, 1, w, p, heads, oa.GLOBAL, 900 + s_len, scale=qscale, rows=rows, lse=True)
+
+
+def test_persistent_kernel_many_items_per_cta(api):
+    # 148 SMs, 6000 work items of 2 KV tiles each: every CTA of the persistent kernel takes ~40 items through cluster launch
+    # control; items with a dead second Q tile (S = 200 < 256... every item here) and live ones (S = 300) interleave per sequence
+    for s_len in (200, 300):
+        q, k, v = synth.qkv(250, s_len, 12, 64, 77 + s_len, device="cuda")
+        out, lse = api.window_attention(q, k, v, 1, s_len, oa.GLOBAL, return_lse=True)
+        again = api.window_attention(q, k, v, 1, s_len, oa.GLOBAL)
+        assert torch.equal(out, again)
+        for n in (0, 123, 249):
+            ref, lse_ref = oa.window_attention(_to64(q[n:n + 1]), _to64(k[n:n + 1]), _to64(v[n:n + 1]), 1, s_len, oa.GLOBAL)
+            d = _to64(out[n:n + 1]) - ref
+            assert np.abs(d).max() <= MAX_ABS and np.linalg.norm(d) / np.linalg.norm(ref) <= REL_L2
+            assert np.abs(lse[n:n + 1].cpu().numpy() - lse_ref).max() <= 4e-3
+
+
 def test_frame_tokens_777(api):
     # the paper-shaped frame: P = 777 = 6*128 + 9 tokens
     _check(api, 1, 2, 777, 2, oa.FRAME, 99, lse=True)
