@@ -465,7 +465,8 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if ((st = cached_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
     const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
     const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
-    if ((seq_len + kBN - 1) / kBN < kPersistentBelowTiles)      // short items: persistent kernel (cluster launch control)
+    // short items: persistent kernel (cluster launch control; its grid is 3-D, so heads and sequences must fit a grid dimension)
+    if ((seq_len + kBN - 1) / kBN < kPersistentBelowTiles && heads <= 65535 && sequences <= 65535)
         return launch_attention_clc(mq, mk, mv, mo, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
     {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
         static std::atomic<bool> attr_set[64];

@@ -462,8 +462,8 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
 mf_status launch_attention_clc(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
                                int sequences, int seq_len, int heads, const AttnParams& prm, cudaStream_t stream) {
     using namespace clc;
-    if (heads > 65535 || sequences > 65535)
-        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: more than 65535 heads or sequences in one launch");
+    if (heads > 65535 || sequences > 65535)       // (the caller keeps such launches on the 1-D grid of attention.cu)
+        return fail(MF_ERR_INVALID_ARG, "launch_attention_clc: heads and sequences must fit a grid dimension");
     const int smem = static_cast<int>(sizeof(Smem)) + 1024;
     {   // the opt-in shared-memory size is a per-device attribute of the kernel: set it once per device
         static std::atomic<bool> attr_set[64];
