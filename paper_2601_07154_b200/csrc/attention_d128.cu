@@ -126,7 +126,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
     const uint32_t tmem = sm.tmem_base;
 
     if (warp >= 8) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         if (warp == 8) {
             // ===================== TMA producer =====================
             if (lane == 0) {
@@ -183,7 +183,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
         }
         if (warp <= 10 && lane == 0) ptx::mbar_arrive(&sm.roles_done);
     } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== softmax warpgroups =====================
         const int tile = warp >> 2;
         if (tile == 0 || tile1_live) {
