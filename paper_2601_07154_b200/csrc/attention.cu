@@ -157,7 +157,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
                     ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
                     ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
-                }
+                                    }
             }
         } else if (warp <= 10) {
             // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================

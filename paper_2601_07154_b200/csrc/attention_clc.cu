@@ -193,7 +193,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
                         ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
                         ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, it.head, j * kBN, it.seq);
-                    }
+                                            }
                     it = fetch_item(sm, qi + 1);
                 }
             }
@@ -277,7 +277,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 }
             }
         } else if (lane == 0) {
-            ptx::watchdog(&sm.roles_done);                // warp 11: traps if the 11 role warps do not finish within seconds
+            ptx::watchdog_progress(&sm.roles_done, sm.k_full);                // warp 11: traps if the 11 role warps do not finish within seconds
         }
         if (warp <= 10 && lane == 0) ptx::mbar_arrive(&sm.roles_done);
     } else {

@@ -145,7 +145,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                     ptx::mbar_arrive_expect_tx(&sm.v_full[st], 2 * kKVHalfBytes);
                     ptx::tma_load_4d(sm.v[st].lo, &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
                     ptx::tma_load_4d(sm.v[st].hi, &map_v, &sm.v_full[st], kDH, head, j * kBN, seq);
-                }
+                                    }
             }
         } else if (warp <= 10) {
             // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================

@@ -50,28 +50,54 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 
 // ---- watchdog ---------------------------------------------------------------------------------
 // Kernels whose warps spin on mbarriers park one otherwise idle warp here.  Every role warp arrives on a "roles done"
-// mbarrier when it leaves its loop; the watchdog waits for that phase with try_wait and a long suspend-time hint (the
-// hardware parks the thread and wakes it when the phase completes, so the CTA is not held back), and traps once
-// kWatchdogNs have passed.  A pipeline-protocol bug (a barrier that never completes) therefore ends the kernel with a
-// CUDA error (MF_ERR_CUDA at the next runtime call) instead of hanging the GPU, at no cost to the waits themselves.
-// A CTA of these kernels lives for microseconds to milliseconds; the limit is seconds.
+// mbarrier when it leaves its loop; the watchdog waits for that phase with try_wait and a 1 ms suspend-time hint (the
+// hardware parks the thread and wakes it when the phase completes, so the CTA is not held back) and traps when the CTA
+// is stuck.  A pipeline-protocol bug (a barrier that never completes) therefore ends the kernel with a CUDA error
+// (MF_ERR_CUDA at the next runtime call) instead of hanging the GPU, at no cost to the waits themselves.
+// Two notions of "stuck":
+//  * watchdog(): the CTA has lived longer than kWatchdogNs.  For kernels whose CTAs live microseconds to a millisecond
+//    (one work item each), so that even a profiler's instrumented replay stays far below the limit.
+//  * watchdog_progress(): the pipeline has not moved for kWatchdogNs.  For persistent CTAs, whose lifetime is the
+//    kernel's: each time the hint runs out it reads the state words of the K-stage "full" barriers (opaque, but they change
+//    with every tile the pipeline moves).  The roles execute nothing for it (a counter bumped by the TMA producer once per
+//    tile was measured: -1 % on the campus launch); it is out of line so that its code does not perturb theirs.
 constexpr unsigned long long kWatchdogNs = 4000000000ull;
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+__device__ __forceinline__ bool watchdog_done(uint64_t* roles_done) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(roles_done)), "r"(0u), "r"(1000000u) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void watchdog(uint64_t* roles_done) {          // one lane of the idle warp
     const unsigned long long t0 = globaltimer_ns();
     for (;;) {
-        uint32_t ok;
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok) : "r"(smem_u32(roles_done)), "r"(0u), "r"(1000000u) : "memory");
-        if (ok) return;
+        if (watchdog_done(roles_done)) return;
         if (globaltimer_ns() - t0 > kWatchdogNs) __trap();
+    }
+}
+template <int N>
+__device__ __noinline__ void watchdog_progress(uint64_t* roles_done, const uint64_t (&stage_bars)[N]) {    // one lane of the idle warp
+    unsigned long long t0 = globaltimer_ns(), seen = 0;
+    for (;;) {
+        if (watchdog_done(roles_done)) return;
+        unsigned long long now = 0;
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            now = now * 0x9E3779B97F4A7C15ull + *reinterpret_cast<const volatile unsigned long long*>(&stage_bars[i]);
+        if (now != seen) {
+            seen = now;
+            t0 = globaltimer_ns();
+        } else if (globaltimer_ns() - t0 > kWatchdogNs) {
+            __trap();
+        }
     }
 }
 
