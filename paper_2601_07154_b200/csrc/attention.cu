@@ -27,6 +27,7 @@
 #include <cuda_bf16.h>
 
 #include <atomic>
+#include <cstddef>
 #include <mutex>
 
 namespace mf {
@@ -69,18 +70,18 @@ constexpr uint32_t kIdescQK = ptx::idesc_bf16_f32(kBM, kBN, 0, 0);
 constexpr uint32_t kIdescPV = ptx::idesc_bf16_f32(kBM, kON, 0, 1);      // V is MN-major ([keys][d], d contiguous)
 
 // S[tile] = Q[tile] K^T : 4 MMAs of K=16 (32-byte steps inside the 128-byte swizzle atom)
-__device__ __forceinline__ void issue_qk(uint32_t tmem_s, const uint8_t* q, const uint8_t* k) {
-    const uint64_t qd = ptx::smem_desc_sw128(ptx::smem_u32(q));
-    const uint64_t kd = ptx::smem_desc_sw128(ptx::smem_u32(k));
+__device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q, uint32_t k) {          // q, k: shared-memory addresses
+    const uint64_t qd = ptx::smem_desc_sw128(q);
+    const uint64_t kd = ptx::smem_desc_sw128(k);
 #pragma unroll
     for (int i = 0; i < kD / 16; ++i) ptx::mma_ss(tmem_s, qd + 2 * i, kd + 2 * i, kIdescQK, i > 0);
 }
 // O[tile] (+)= P_half[tile] V_half : 4 MMAs of K=16 keys; P slice = 8 TMEM columns, V slice = 16 rows = 2048 B
 // v_half points at the first of the 64 key rows.  B = [V | ones]: atom 0 = the V rows, atom 1 (columns 64..79) =
 // the same rows of the ones tile, LBO bytes further on.
-__device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, const uint8_t* v_half, uint32_t ones_minus_v,
+__device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_half, uint32_t ones_minus_v,
                                               bool accumulate) {
-    const uint64_t vd = ptx::smem_desc_sw128(ptx::smem_u32(v_half), ones_minus_v);
+    const uint64_t vd = ptx::smem_desc_sw128(v_half, ones_minus_v);
 #pragma unroll
     for (int i = 0; i < kBN / 32; ++i)
         ptx::mma_ts(tmem_o, tmem_p + 8 * i, vd + (2048 >> 4) * i, kIdescPV, (accumulate || i > 0) ? 1u : 0u);
@@ -145,53 +146,60 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
         if (warp == 8) {
             // ===================== TMA producer =====================
             if (lane == 0) {
-                ptx::mbar_arrive_expect_tx(&sm.q_full, (tile1_live ? 2 : 1) * kTileBytes);
-                ptx::tma_load_4d(sm.q[0], &map_q, &sm.q_full, 0, head, row0, seq);
-                if (tile1_live) ptx::tma_load_4d(sm.q[1], &map_q, &sm.q_full, 0, head, row0 + kBM, seq);
+                const uint32_t sb = ptx::smem_base_u32(&sm);          // addresses = one opaque base register + constants
+                const uint32_t a_q_full = sb + offsetof(AttnSmem, q_full);
+                ptx::mbar_arrive_expect_tx(a_q_full, (tile1_live ? 2 : 1) * kTileBytes);
+                ptx::tma_load_4d(sb + offsetof(AttnSmem, q), &map_q, a_q_full, 0, head, row0, seq);
+                if (tile1_live) ptx::tma_load_4d(sb + offsetof(AttnSmem, q) + kTileBytes, &map_q, a_q_full, 0, head, row0 + kBM, seq);
                 for (int j = 0; j < n_kv; ++j) {
                     const int st = j % kStages;
                     const uint32_t ph = (j / kStages) & 1;
-                    ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
-                    ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
-                    ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, head, j * kBN, seq);
-                    ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
-                    ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
-                    ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
-                                    }
+                    ptx::mbar_wait(sb + offsetof(AttnSmem, k_empty) + 8 * st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(sb + offsetof(AttnSmem, k_full) + 8 * st, kTileBytes);
+                    ptx::tma_load_4d(sb + offsetof(AttnSmem, k) + kTileBytes * st, &map_k, sb + offsetof(AttnSmem, k_full) + 8 * st, 0, head, j * kBN, seq);
+                    ptx::mbar_wait(sb + offsetof(AttnSmem, v_empty) + 8 * st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(sb + offsetof(AttnSmem, v_full) + 8 * st, kTileBytes);
+                    ptx::tma_load_4d(sb + offsetof(AttnSmem, v) + kTileBytes * st, &map_v, sb + offsetof(AttnSmem, v_full) + 8 * st, 0, head, j * kBN, seq);
+                }
             }
         } else if (warp <= 10) {
             // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================
             const int t = warp - 9;
             if (lane == 0 && (t == 0 || tile1_live)) {
                 const uint32_t t_s = tmem + kColS + t * kBN, t_o = tmem + kColO + t * kON, t_p = tmem + kColP + t * kPH;
-                ptx::mbar_wait(&sm.q_full, 0);
-                ptx::mbar_wait(&sm.k_full[0], 0);
+                const uint32_t sb = ptx::smem_base_u32(&sm);          // addresses = one opaque base register + constants
+                const uint32_t a_q = sb + offsetof(AttnSmem, q) + kTileBytes * t, a_k = sb + offsetof(AttnSmem, k), a_v = sb + offsetof(AttnSmem, v);
+                const uint32_t a_ones = sb + offsetof(AttnSmem, ones);
+                const uint32_t a_s_full = sb + offsetof(AttnSmem, s_full) + 8 * t, a_s_free = sb + offsetof(AttnSmem, s_free) + 8 * t;
+                const uint32_t a_p_full = sb + offsetof(AttnSmem, p_full) + 8 * t, a_pv_done = sb + offsetof(AttnSmem, pv_done) + 8 * t;
+                ptx::mbar_wait(sb + offsetof(AttnSmem, q_full), 0);
+                ptx::mbar_wait(sb + offsetof(AttnSmem, k_full), 0);
                 ptx::tc_fence_after();
-                issue_qk(t_s, sm.q[t], sm.k[0]);
-                ptx::mma_commit(&sm.s_full[t]);
-                ptx::mma_commit(&sm.k_empty[0]);
+                issue_qk(t_s, a_q, a_k);
+                ptx::mma_commit(a_s_full);
+                ptx::mma_commit(sb + offsetof(AttnSmem, k_empty));
                 for (int j = 0; j < n_kv; ++j) {
                     const int st = j % kStages;
                     if (j + 1 < n_kv) {
                         // S(j+1) as soon as the softmax warpgroup holds S(j) in registers
                         const int st1 = (j + 1) % kStages;
-                        ptx::mbar_wait(&sm.s_free[t], j & 1);
-                        ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
+                        ptx::mbar_wait(a_s_free, j & 1);
+                        ptx::mbar_wait(sb + offsetof(AttnSmem, k_full) + 8 * st1, ((j + 1) / kStages) & 1);
                         ptx::tc_fence_after();
-                        issue_qk(t_s, sm.q[t], sm.k[st1]);
-                        ptx::mma_commit(&sm.s_full[t]);
-                        ptx::mma_commit(&sm.k_empty[st1]);
+                        issue_qk(t_s, a_q, a_k + kTileBytes * st1);
+                        ptx::mma_commit(a_s_full);
+                        ptx::mma_commit(sb + offsetof(AttnSmem, k_empty) + 8 * st1);
                     }
-                    ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
-                    const uint32_t ones_minus_v = ptx::smem_u32(sm.ones) - ptx::smem_u32(sm.v[st]);
+                    ptx::mbar_wait(sb + offsetof(AttnSmem, v_full) + 8 * st, (j / kStages) & 1);
+                    const uint32_t v_st = a_v + kTileBytes * st;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        ptx::mbar_wait(&sm.p_full[h][t], j & 1);
+                        ptx::mbar_wait(a_p_full + 8 * kQTiles * h, j & 1);
                         ptx::tc_fence_after();
-                        issue_pv_half(t_o, t_p, sm.v[st] + h * (kTileBytes / 2), ones_minus_v, j > 0 || h > 0);
-                        ptx::mma_commit(&sm.pv_done[h][t]);
+                        issue_pv_half(t_o, t_p, v_st + h * (kTileBytes / 2), a_ones - v_st, j > 0 || h > 0);
+                        ptx::mma_commit(a_pv_done + 8 * kQTiles * h);
                     }
-                    ptx::mma_commit(&sm.v_empty[st]);
+                    ptx::mma_commit(sb + offsetof(AttnSmem, v_empty) + 8 * st);
                 }
             }
         } else if (lane == 0) {
@@ -210,8 +218,13 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const uint32_t t_p = tmem + lane_addr + kColP + tile * kPH;
             float m_used = -INFINITY;                     // running max in scaled log2 units
             const uint64_t scale2 = ptx::pack2(prm.scale_log2, prm.scale_log2);
+            // barrier addresses = one opaque base register + constants (see smem_base_u32)
+            const uint32_t sb = ptx::smem_base_u32(&sm);
+            const uint32_t a_s_full = sb + offsetof(AttnSmem, s_full) + 8 * tile, a_s_free = sb + offsetof(AttnSmem, s_free) + 8 * tile;
+            const uint32_t a_p_full0 = sb + offsetof(AttnSmem, p_full) + 8 * tile, a_p_full1 = a_p_full0 + 8 * kQTiles;
+            const uint32_t a_pv_done0 = sb + offsetof(AttnSmem, pv_done) + 8 * tile, a_pv_done1 = a_pv_done0 + 8 * kQTiles;
             for (int j = 0; j < n_kv; ++j) {
-                ptx::mbar_wait(&sm.s_full[tile], j & 1);
+                ptx::mbar_wait(a_s_full, j & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
 #pragma unroll
@@ -220,9 +233,9 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 ptx::tc_fence_before();
                 __syncwarp();
 #ifdef MF_TEST_PROTOCOL_BUG      // test builds only (tests/test_gpu_watchdog.py): CTA 0 never hands S back, so its pipeline stalls for good
-                if (lane == 0 && blockIdx.x != 0) ptx::mbar_arrive(&sm.s_free[tile]);
+                if (lane == 0 && blockIdx.x != 0) ptx::mbar_arrive(a_s_free);
 #else
-                if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by S(j+1)
+                if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by S(j+1)
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
@@ -251,7 +264,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, grow)) {
                     // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
-                    ptx::mbar_wait(&sm.pv_done[1][tile], (j - 1) & 1);
+                    ptx::mbar_wait(a_pv_done1, (j - 1) & 1);
                     ptx::tc_fence_after();
                     const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
                     if (grow) m_used = m_new;
@@ -293,26 +306,26 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                         pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1]));
                     }
                     // the P half buffer is free once the previous PV that read it has completed
-                    if (h == 1) ptx::mbar_wait(&sm.pv_done[0][tile], j & 1);
-                    else if (j > 0) ptx::mbar_wait(&sm.pv_done[1][tile], (j - 1) & 1);
+                    if (h == 1) ptx::mbar_wait(a_pv_done0, j & 1);
+                    else if (j > 0) ptx::mbar_wait(a_pv_done1, (j - 1) & 1);
                     ptx::tc_fence_after();
                     ptx::tmem_st32(t_p, pk);
                     ptx::tc_wait_st();
                     ptx::tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&sm.p_full[h][tile]);
+                    if (lane == 0) ptx::mbar_arrive(h ? a_p_full1 : a_p_full0);
                     if (h == 0) {
                         // Keep the second half's exponentials behind the first half's store (ptxas would hoist them
                         // above it): their scale operand passes through an opaque shared-memory read of a zero word.
                         uint32_t z;
-                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(ptx::smem_u32(&sm.zero)) : "memory");
+                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(sb + static_cast<uint32_t>(offsetof(AttnSmem, zero))) : "memory");
                         scale_h = ptx::pack2(__uint_as_float(__float_as_uint(prm.scale_log2) | z),
                                              __uint_as_float(__float_as_uint(prm.scale_log2) | z));
                     }
                 }
             }
             // ---- epilogue: O / l -> bf16 -> global ----
-            ptx::mbar_wait(&sm.pv_done[1][tile], (n_kv - 1) & 1);
+            ptx::mbar_wait(a_pv_done1, (n_kv - 1) & 1);
             ptx::tc_fence_after();
             const int row = row0 + tile * kBM + row_in_tile;
             uint32_t o[2][32];

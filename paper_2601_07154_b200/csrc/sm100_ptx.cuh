@@ -48,6 +48,39 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     }
 }
 
+// The same operations on a 32-bit shared-memory address.  A role loop forms `base + offsetof(field)` from one opaque base
+// register (smem_base_u32): taking `&sm.field` of the 1024-byte-aligned view of dynamic shared memory instead makes the
+// compiler rebuild that view (a dozen instructions with the shared window's base) at every barrier operation.
+__device__ __forceinline__ uint32_t smem_base_u32(const void* p) {
+    uint32_t a = smem_u32(p), r;
+    asm volatile("mov.u32 %0, %1;" : "=r"(r) : "r"(a));          // opaque: kept in a register, not rematerialised
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t smem_dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        :: "r"(smem_dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+
 // ---- watchdog ---------------------------------------------------------------------------------
 // Kernels whose warps spin on mbarriers park one otherwise idle warp here.  Every role warp arrives on a "roles done"
 // mbarrier when it leaves its loop; the watchdog waits for that phase with try_wait and a 1 ms suspend-time hint (the
