@@ -18,6 +18,7 @@
 #include "tensormap.h"
 
 #include <atomic>
+#include <cstddef>
 
 namespace mf {
 namespace clc {
@@ -290,6 +291,11 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
         const uint32_t t_o = tmem + lane_addr + kColO + tile * kON;
         const uint32_t t_p = tmem + lane_addr + kColP + tile * kPH;
         const uint64_t scale2 = ptx::pack2(prm.scale_log2, prm.scale_log2);
+        // barrier addresses = one opaque base register + constants (sm100_ptx.cuh: smem_base_u32)
+        const uint32_t sb = ptx::smem_base_u32(&sm);
+        const uint32_t a_s_full = sb + offsetof(Smem, s_full) + 8 * tile, a_s_free = sb + offsetof(Smem, s_free) + 8 * tile;
+        const uint32_t a_p_full0 = sb + offsetof(Smem, p_full) + 8 * tile, a_p_full1 = a_p_full0 + 8 * kQTiles;
+        const uint32_t a_pv_done0 = sb + offsetof(Smem, pv_done) + 8 * tile, a_pv_done1 = a_pv_done0 + 8 * kQTiles;
         uint32_t ns = 0;                                  // KV tiles consumed by this warpgroup (phase counter, runs across items)
         int store_pending = -1;                           // (thread row_in_tile == 0) Q slot whose output store is still reading shared memory
         Item it = own_item();
@@ -306,7 +312,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
             }
             float m_used = -INFINITY;                     // running max in scaled log2 units
             for (int j = 0; j < n_kv; ++j, ++ns) {
-                ptx::mbar_wait(&sm.s_full[tile], ns & 1);
+                ptx::mbar_wait(a_s_full, ns & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
 #pragma unroll
@@ -315,9 +321,9 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 ptx::tc_fence_before();
                 __syncwarp();
 #ifdef MF_TEST_PROTOCOL_BUG      // test builds only (tests/test_gpu_watchdog.py): CTA (0,0,0) never hands S back, so its pipeline stalls for good
-                if (lane == 0 && (blockIdx.x | blockIdx.y | blockIdx.z) != 0) ptx::mbar_arrive(&sm.s_free[tile]);
+                if (lane == 0 && (blockIdx.x | blockIdx.y | blockIdx.z) != 0) ptx::mbar_arrive(a_s_free);
 #else
-                if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by the next S
+                if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by the next S
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
@@ -342,7 +348,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, grow)) {
                     // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
-                    ptx::mbar_wait(&sm.pv_done[1][tile], (ns - 1) & 1);
+                    ptx::mbar_wait(a_pv_done1, (ns - 1) & 1);
                     ptx::tc_fence_after();
                     const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
                     if (grow) m_used = m_new;
@@ -384,19 +390,19 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1]));
                     }
                     // the P half buffer is free once the previous PV that read it has completed
-                    if (h == 1) ptx::mbar_wait(&sm.pv_done[0][tile], ns & 1);
-                    else if (ns > 0) ptx::mbar_wait(&sm.pv_done[1][tile], (ns - 1) & 1);
+                    if (h == 1) ptx::mbar_wait(a_pv_done0, ns & 1);
+                    else if (ns > 0) ptx::mbar_wait(a_pv_done1, (ns - 1) & 1);
                     ptx::tc_fence_after();
                     ptx::tmem_st32(t_p, pk);
                     ptx::tc_wait_st();
                     ptx::tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&sm.p_full[h][tile]);
+                    if (lane == 0) ptx::mbar_arrive(h ? a_p_full1 : a_p_full0);
                     if (h == 0) {
                         // Keep the second half's exponentials behind the first half's store (ptxas would hoist them
                         // above it): their scale operand passes through an opaque shared-memory read of a zero word.
                         uint32_t z;
-                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(ptx::smem_u32(&sm.zero)) : "memory");
+                        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(z) : "r"(sb + static_cast<uint32_t>(offsetof(Smem, zero))) : "memory");
                         scale_h = ptx::pack2(__uint_as_float(__float_as_uint(prm.scale_log2) | z),
                                              __uint_as_float(__float_as_uint(prm.scale_log2) | z));
                     }
@@ -409,7 +415,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 }
             }
             // ---- epilogue: O / l -> bf16 -> shared memory (this item's Q tile) -> one TMA store ----
-            ptx::mbar_wait(&sm.pv_done[1][tile], (ns - 1) & 1);
+            ptx::mbar_wait(a_pv_done1, (ns - 1) & 1);
             ptx::tc_fence_after();
             const int row = it.row0() + tile * kBM + row_in_tile;
             uint32_t o[2][32];
