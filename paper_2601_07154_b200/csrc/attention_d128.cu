@@ -15,6 +15,7 @@
 #include "tensormap.h"
 
 #include <atomic>
+#include <cstddef>
 
 namespace mf {
 namespace d128 {
@@ -194,8 +195,12 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
             const uint32_t t_p = tmem + lane_addr + kColP + tile * kPCols;
             float m_used = -INFINITY;                     // running max in scaled log2 units
             const uint64_t scale2 = ptx::pack2(prm.scale_log2, prm.scale_log2);
+            // barrier addresses = one opaque base register + constants (sm100_ptx.cuh: smem_base_u32)
+            const uint32_t sb = ptx::smem_base_u32(&sm);
+            const uint32_t a_s_full = sb + offsetof(Smem, s_full) + 8 * tile, a_s_free = sb + offsetof(Smem, s_free) + 8 * tile;
+            const uint32_t a_p_full = sb + offsetof(Smem, p_full) + 8 * tile, a_pv_done = sb + offsetof(Smem, pv_done) + 8 * tile;
             for (int j = 0; j < n_kv; ++j) {
-                ptx::mbar_wait(&sm.s_full[tile], j & 1);
+                ptx::mbar_wait(a_s_full, j & 1);
                 ptx::tc_fence_after();
                 uint32_t s[2][32];
                 ptx::tmem_ld32(t_s, s[0]);
@@ -203,7 +208,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                 ptx::tc_wait_ld();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(&sm.s_free[tile]);       // S columns may be overwritten by S(j+1)
+                if (lane == 0) ptx::mbar_arrive(a_s_free);       // S columns may be overwritten by S(j+1)
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
                 if (valid < kBN) {
 #pragma unroll
@@ -227,7 +232,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, grow)) {
                     // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
-                    ptx::mbar_wait(&sm.pv_done[tile], (j - 1) & 1);
+                    ptx::mbar_wait(a_pv_done, (j - 1) & 1);
                     ptx::tc_fence_after();
                     const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
                     if (grow) m_used = m_new;
@@ -266,16 +271,16 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                     pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[1][2 * i]), __uint_as_float(s[1][2 * i + 1]));
                 }
                 // the P buffer is free once PV(j-1), which read it, has completed
-                if (j > 0) ptx::mbar_wait(&sm.pv_done[tile], (j - 1) & 1);
+                if (j > 0) ptx::mbar_wait(a_pv_done, (j - 1) & 1);
                 ptx::tc_fence_after();
                 ptx::tmem_st32(t_p, pk);
                 ptx::tc_wait_st();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(&sm.p_full[tile]);
+                if (lane == 0) ptx::mbar_arrive(a_p_full);
             }
             // ---- epilogue: O / l -> bf16 -> global ----
-            ptx::mbar_wait(&sm.pv_done[tile], (n_kv - 1) & 1);
+            ptx::mbar_wait(a_pv_done, (n_kv - 1) & 1);
             ptx::tc_fence_after();
             const int row = row0 + tile * kBM + row_in_tile;
             const float l = __uint_as_float(ptx::tmem_ld1(t_o + kD));           // row sum from the ones column
