@@ -255,9 +255,14 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         } else {
                             ptx::mma_commit(&sm.q_empty[slot]);             // every Q K^T of this item has been issued
                             next = fetch_item(sm, qi + 1);  // (asked for when this item began: long since answered)
-                            if (next.valid && (t == 0 || next.tile1_live(prm))) {
-                                ptx::mbar_wait(&sm.q_full[slot ^ 1], ((qi + 1) >> 1) & 1);
-                                issue_s(slot ^ 1, kv + 1);  // the next item's S(0), ahead of this item's last P V
+                            // The next item's S(0), ahead of this item's last P V -- but only if its Q tiles have landed: this
+                            // thread must never BLOCK on the future while it still owes the present its P V.  (With one KV tile
+                            // per item the next-but-one Q load waits for this item's output store, which waits for the softmax
+                            // warps, which wait for this P V: a blocking wait here deadlocked S <= 128 launches of more than
+                            // 148 items; found by differential fuzzing against attention.cu, ended by the watchdog.)
+                            if (next.valid && (t == 0 || next.tile1_live(prm)) &&
+                                ptx::mbar_try_wait(&sm.q_full[slot ^ 1], ((qi + 1) >> 1) & 1)) {
+                                issue_s(slot ^ 1, kv + 1);
                                 have_s = true;
                             }
                         }
