@@ -307,3 +307,47 @@ def test_errors(api):
         api.window_attention(q, k, v, 2, 30)                       # S mismatch
     with pytest.raises(api.MfError):
         api.window_attention(q, k, v, 1, 64, out=q)                # aliasing
+
+
+def test_concurrent_streams_graph_replay_and_many_items(api):
+    # the persistent kernel takes its work from the hardware's launch queue (cluster launch control): two of them and a long
+    # one-item-per-CTA launch running at once on three streams, the same launches replayed from a CUDA graph, and a launch of
+    # 60000 two-tile items must all reproduce the serial results bit for bit
+    a = synth.qkv(6, 8 * 300, 8, 64, 1, device="cuda")
+    b = synth.qkv(3, 16 * 129, 12, 64, 2, device="cuda")
+    c = synth.qkv(2, 9000, 4, 64, 3, device="cuda")
+    ref_a = api.window_attention(*a, 8, 300, oa.FRAME)
+    ref_b = api.window_attention(*b, 16, 129, oa.FRAME)
+    ref_c = api.window_attention(*c, 1, 9000, oa.GLOBAL)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    for _ in range(10):
+        with torch.cuda.stream(streams[0]):
+            out_a = api.window_attention(*a, 8, 300, oa.FRAME)
+        with torch.cuda.stream(streams[1]):
+            out_b = api.window_attention(*b, 16, 129, oa.FRAME)
+        with torch.cuda.stream(streams[2]):
+            out_c = api.window_attention(*c, 1, 9000, oa.GLOBAL)
+        torch.cuda.synchronize()
+        assert torch.equal(out_a, ref_a) and torch.equal(out_b, ref_b) and torch.equal(out_c, ref_c)
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    out_a, out_c = torch.empty_like(a[0]), torch.empty_like(c[0])
+    with torch.cuda.stream(side):
+        api.window_attention(*a, 8, 300, oa.FRAME, out=out_a)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            for _ in range(3):
+                api.window_attention(*a, 8, 300, oa.FRAME, out=out_a)
+                api.window_attention(*c, 1, 9000, oa.GLOBAL, out=out_c)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(5):
+        out_a.zero_()
+        out_c.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out_a, ref_a) and torch.equal(out_c, ref_c)
+    q, k, v = synth.qkv(2500, 200, 24, 64, 5, device="cuda")
+    first = api.window_attention(q, k, v, 1, 200)
+    again = api.window_attention(q, k, v, 1, 200)
+    assert torch.equal(first, again) and torch.isfinite(first.float()).all()
