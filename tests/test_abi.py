@@ -88,3 +88,25 @@ def test_missing_library_fails_loudly(monkeypatch):
     monkeypatch.setattr(api, "LIB_PATH", "/nonexistent/libmf_b200.so")
     with pytest.raises(api.MfError):
         api.lib()
+
+
+def test_binding_window_starts_and_synth_take_them_as_input():
+    # the window partition (step a1) is never computed by the input generator: it takes the starts it is given
+    import numpy as np
+    import pytest
+    from oracle import windows as ow
+    from paper_2601_07154_b200 import api, synth
+    assert api.window_starts(1800, 32, 16) == ow.window_starts(1800, 32, 16)
+    assert api.window_starts(11, 4, 3) == [0, 3, 6, 7]
+    with pytest.raises(api.MfError):
+        api.window_starts(3, 4, 2)
+    traj = synth.trajectory(synth.CONFIGS[1], 7, 11)
+    loc = synth.local_windows(traj, 4, [0, 3, 6, 7])
+    assert loc.shape == (4, 4, 4, 4)
+    for i, s0 in enumerate([0, 3, 6, 7]):                  # window-local gauge: the window's first pose is the identity
+        assert np.allclose(loc[i, 0], np.eye(4), atol=1e-6)
+        assert np.allclose(loc[i, 3], (traj[s0 + 3] @ np.linalg.inv(traj[s0])).astype(np.float32), atol=1e-6)
+    custom = synth.local_windows(traj, 4, [5])             # any caller-chosen start works: no partition logic inside
+    assert custom.shape == (1, 4, 4, 4)
+    d, g = synth.depth_windows(11, 4, [0, 3, 6, 7], 6, 8, 3)
+    assert d.shape == (4, 4, 6, 8) and g.shape == (4,)
