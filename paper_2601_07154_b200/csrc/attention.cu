@@ -29,6 +29,7 @@
 #include <atomic>
 #include <cstddef>
 #include <mutex>
+#include <type_traits>
 
 namespace mf {
 
@@ -223,7 +224,9 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const uint32_t a_s_full = sb + offsetof(AttnSmem, s_full) + 8 * tile, a_s_free = sb + offsetof(AttnSmem, s_free) + 8 * tile;
             const uint32_t a_p_full0 = sb + offsetof(AttnSmem, p_full) + 8 * tile, a_p_full1 = a_p_full0 + 8 * kQTiles;
             const uint32_t a_pv_done0 = sb + offsetof(AttnSmem, pv_done) + 8 * tile, a_pv_done1 = a_pv_done0 + 8 * kQTiles;
-            for (int j = 0; j < n_kv; ++j) {
+            // One KV tile.  The loop below runs it without the tail-masking code (hundreds of selects that only a ragged LAST tile
+            // needs: peeled off, the steady-state loop is one contiguous block of code); the last tile picks its instantiation.
+            auto kv_tile = [&](const int j, auto masked) {
                 ptx::mbar_wait(a_s_full, j & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
@@ -238,7 +241,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by S(j+1)
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
-                if (valid < kBN) {
+                if (decltype(masked)::value) {
 #pragma unroll
                     for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -323,7 +326,10 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                                              __uint_as_float(__float_as_uint(prm.scale_log2) | z));
                     }
                 }
-            }
+            };
+            for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::false_type{});
+            if (prm.seq_len % kBN != 0) kv_tile(n_kv - 1, std::true_type{});
+            else kv_tile(n_kv - 1, std::false_type{});
             // ---- epilogue: O / l -> bf16 -> global ----
             ptx::mbar_wait(a_pv_done1, (n_kv - 1) & 1);
             ptx::tc_fence_after();
