@@ -19,6 +19,7 @@
 
 #include <atomic>
 #include <cstddef>
+#include <type_traits>
 
 namespace mf {
 namespace clc {
@@ -316,7 +317,9 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 continue;
             }
             float m_used = -INFINITY;                     // running max in scaled log2 units
-            for (int j = 0; j < n_kv; ++j, ++ns) {
+            // One KV tile.  The loop below runs it without the tail-masking code (only a ragged LAST tile needs it: peeled off, the
+            // steady-state loop is one contiguous block of code); the last tile picks its instantiation.
+            auto kv_tile = [&](const int j, auto masked) {
                 ptx::mbar_wait(a_s_full, ns & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
@@ -331,7 +334,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by the next S
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
-                if (valid < kBN) {
+                if (decltype(masked)::value) {
 #pragma unroll
                     for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -418,7 +421,11 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     ptx::mbar_arrive(&sm.q_empty[store_pending]);
                     store_pending = -1;
                 }
-            }
+            };
+            for (int j = 0; j + 1 < n_kv; ++j, ++ns) kv_tile(j, std::false_type{});
+            if (prm.seq_len % kBN != 0) kv_tile(n_kv - 1, std::true_type{});
+            else kv_tile(n_kv - 1, std::false_type{});
+            ++ns;
             // ---- epilogue: O / l -> bf16 -> shared memory (this item's Q tile) -> one TMA store ----
             ptx::mbar_wait(a_pv_done1, (ns - 1) & 1);
             ptx::tc_fence_after();
