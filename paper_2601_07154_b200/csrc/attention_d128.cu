@@ -16,6 +16,7 @@
 
 #include <atomic>
 #include <cstddef>
+#include <type_traits>
 
 namespace mf {
 namespace d128 {
@@ -199,7 +200,8 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
             const uint32_t sb = ptx::smem_base_u32(&sm);
             const uint32_t a_s_full = sb + offsetof(Smem, s_full) + 8 * tile, a_s_free = sb + offsetof(Smem, s_free) + 8 * tile;
             const uint32_t a_p_full = sb + offsetof(Smem, p_full) + 8 * tile, a_pv_done = sb + offsetof(Smem, pv_done) + 8 * tile;
-            for (int j = 0; j < n_kv; ++j) {
+            // One KV tile; the ragged last tile is peeled off the loop (the steady-state loop holds no tail-masking code).
+            auto kv_tile = [&](const int j, auto masked) {
                 ptx::mbar_wait(a_s_full, j & 1);
                 ptx::tc_fence_after();
                 uint32_t s[2][32];
@@ -210,7 +212,7 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(a_s_free);       // S columns may be overwritten by S(j+1)
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
-                if (valid < kBN) {
+                if (decltype(masked)::value) {
 #pragma unroll
                     for (int c = 0; c < 2; ++c)
 #pragma unroll
@@ -278,7 +280,10 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(a_p_full);
-            }
+            };
+            for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::false_type{});
+            if (prm.seq_len % kBN != 0) kv_tile(n_kv - 1, std::true_type{});
+            else kv_tile(n_kv - 1, std::false_type{});
             // ---- epilogue: O / l -> bf16 -> global ----
             ptx::mbar_wait(a_pv_done, (n_kv - 1) & 1);
             ptx::tc_fence_after();
