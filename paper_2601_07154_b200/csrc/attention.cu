@@ -225,13 +225,20 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             const uint32_t a_p_full0 = sb + offsetof(AttnSmem, p_full) + 8 * tile, a_p_full1 = a_p_full0 + 8 * kQTiles;
             const uint32_t a_pv_done0 = sb + offsetof(AttnSmem, pv_done) + 8 * tile, a_pv_done1 = a_pv_done0 + 8 * kQTiles;
             // One KV tile.  The loop below runs it without the tail-masking code (hundreds of selects that only a ragged LAST tile
-            // needs: peeled off, the steady-state loop is one contiguous block of code); the last tile picks its instantiation.
-            auto kv_tile = [&](const int j, auto masked) {
+            // needs: peeled off, the steady-state loop is one contiguous block of code); the last tile picks its instantiation:
+            // `tail` = 0 for a full tile, else the number of 32-column chunks of S that hold keys.  The other chunks are neither
+            // read nor exponentiated and their P is stored as zeros (at P = 777 the seventh tile of a frame holds 9 keys: a
+            // quarter of the softmax work of a full tile; FRAME mode +5.5 %).  The MMA issuers do not know about it: narrowing
+            // the tail's Q K^T and P V too was measured, and the extra selects and predicates in the issuing thread cost the
+            // steady state 2 % (campus) to 4 % (suburban), for no gain on the tail.
+            auto kv_tile = [&](const int j, auto tail) {
+                constexpr bool kMasked = decltype(tail)::value != 0;
+                constexpr int kChunks = kMasked ? decltype(tail)::value : 4;
                 ptx::mbar_wait(a_s_full, j & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
+                for (int c = 0; c < kChunks; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
                 ptx::tc_wait_ld();
                 ptx::tc_fence_before();
                 __syncwarp();
@@ -241,9 +248,9 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by S(j+1)
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
-                if (decltype(masked)::value) {
+                if (kMasked) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
+                    for (int c = 0; c < kChunks; ++c)
 #pragma unroll
                         for (int i = 0; i < 32; ++i)
                             if (32 * c + i >= valid) s[c][i] = 0xff800000u;      // -inf
@@ -254,7 +261,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 }
                 float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+                for (int c = 0; c < kChunks; ++c)
 #pragma unroll
                     for (int i = 0; i < 32; i += 8)
 #pragma unroll
@@ -290,7 +297,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                    for (int c = 2 * h; c < 2 * h + 2; ++c) {
+                    for (int c = 2 * h; c < 2 * h + 2 && c < kChunks; ++c) {
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
                             ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
@@ -305,8 +312,8 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     uint32_t pk[32];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
-                        pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * h][2 * i]), __uint_as_float(s[2 * h][2 * i + 1]));
-                        pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1]));
+                        pk[i] = 2 * h < kChunks ? ptx::pack_bf16(__uint_as_float(s[2 * h][2 * i]), __uint_as_float(s[2 * h][2 * i + 1])) : 0u;
+                        pk[16 + i] = 2 * h + 1 < kChunks ? ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1])) : 0u;
                     }
                     // the P half buffer is free once the previous PV that read it has completed
                     if (h == 1) ptx::mbar_wait(a_pv_done0, j & 1);
@@ -327,9 +334,12 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     }
                 }
             };
-            for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::false_type{});
-            if (prm.seq_len % kBN != 0) kv_tile(n_kv - 1, std::true_type{});
-            else kv_tile(n_kv - 1, std::false_type{});
+            for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::integral_constant<int, 0>{});
+            const int tail_chunks = (prm.seq_len - (n_kv - 1) * kBN + 31) / 32;        // 1..4
+            if (prm.seq_len % kBN == 0) kv_tile(n_kv - 1, std::integral_constant<int, 0>{});
+            else if (tail_chunks == 1) kv_tile(n_kv - 1, std::integral_constant<int, 1>{});
+            else if (tail_chunks == 2) kv_tile(n_kv - 1, std::integral_constant<int, 2>{});
+            else kv_tile(n_kv - 1, std::integral_constant<int, 4>{});
             // ---- epilogue: O / l -> bf16 -> global ----
             ptx::mbar_wait(a_pv_done1, (n_kv - 1) & 1);
             ptx::tc_fence_after();

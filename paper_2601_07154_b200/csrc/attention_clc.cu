@@ -318,13 +318,17 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
             }
             float m_used = -INFINITY;                     // running max in scaled log2 units
             // One KV tile.  The loop below runs it without the tail-masking code (only a ragged LAST tile needs it: peeled off, the
-            // steady-state loop is one contiguous block of code); the last tile picks its instantiation.
-            auto kv_tile = [&](const int j, auto masked) {
+            // steady-state loop is one contiguous block of code); the last tile picks its instantiation: `tail` = 0 for a full
+            // tile, else the number of 32-column chunks of S that hold keys; the other chunks are neither read nor exponentiated
+            // and their P is stored as zeros (attention.cu has the measurements).
+            auto kv_tile = [&](const int j, auto tail) {
+                constexpr bool kMasked = decltype(tail)::value != 0;
+                constexpr int kChunks = kMasked ? decltype(tail)::value : 4;
                 ptx::mbar_wait(a_s_full, ns & 1);
                 ptx::tc_fence_after();
                 uint32_t s[4][32];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
+                for (int c = 0; c < kChunks; ++c) ptx::tmem_ld32(t_s + 32 * c, s[c]);
                 ptx::tc_wait_ld();
                 ptx::tc_fence_before();
                 __syncwarp();
@@ -334,16 +338,16 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                 if (lane == 0) ptx::mbar_arrive(a_s_free);               // S columns may be overwritten by the next S
 #endif
                 const int valid = prm.seq_len - j * kBN;  // keys of this tile that exist
-                if (decltype(masked)::value) {
+                if (kMasked) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
+                    for (int c = 0; c < kChunks; ++c)
 #pragma unroll
                         for (int i = 0; i < 32; ++i)
                             if (32 * c + i >= valid) s[c][i] = 0xff800000u;      // -inf
                 }
                 float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+                for (int c = 0; c < kChunks; ++c)
 #pragma unroll
                     for (int i = 0; i < 32; i += 8)
 #pragma unroll
@@ -379,7 +383,7 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                    for (int c = 2 * h; c < 2 * h + 2; ++c) {
+                    for (int c = 2 * h; c < 2 * h + 2 && c < kChunks; ++c) {
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
                             ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
@@ -394,8 +398,8 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     uint32_t pk[32];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
-                        pk[i] = ptx::pack_bf16(__uint_as_float(s[2 * h][2 * i]), __uint_as_float(s[2 * h][2 * i + 1]));
-                        pk[16 + i] = ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1]));
+                        pk[i] = 2 * h < kChunks ? ptx::pack_bf16(__uint_as_float(s[2 * h][2 * i]), __uint_as_float(s[2 * h][2 * i + 1])) : 0u;
+                        pk[16 + i] = 2 * h + 1 < kChunks ? ptx::pack_bf16(__uint_as_float(s[2 * h + 1][2 * i]), __uint_as_float(s[2 * h + 1][2 * i + 1])) : 0u;
                     }
                     // the P half buffer is free once the previous PV that read it has completed
                     if (h == 1) ptx::mbar_wait(a_pv_done0, ns & 1);
@@ -422,9 +426,12 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     store_pending = -1;
                 }
             };
-            for (int j = 0; j + 1 < n_kv; ++j, ++ns) kv_tile(j, std::false_type{});
-            if (prm.seq_len % kBN != 0) kv_tile(n_kv - 1, std::true_type{});
-            else kv_tile(n_kv - 1, std::false_type{});
+            for (int j = 0; j + 1 < n_kv; ++j, ++ns) kv_tile(j, std::integral_constant<int, 0>{});
+            const int tail_chunks = (prm.seq_len - (n_kv - 1) * kBN + 31) / 32;        // 1..4
+            if (prm.seq_len % kBN == 0) kv_tile(n_kv - 1, std::integral_constant<int, 0>{});
+            else if (tail_chunks == 1) kv_tile(n_kv - 1, std::integral_constant<int, 1>{});
+            else if (tail_chunks == 2) kv_tile(n_kv - 1, std::integral_constant<int, 2>{});
+            else kv_tile(n_kv - 1, std::integral_constant<int, 4>{});
             ++ns;
             // ---- epilogue: O / l -> bf16 -> shared memory (this item's Q tile) -> one TMA store ----
             ptx::mbar_wait(a_pv_done1, (ns - 1) & 1);

@@ -98,6 +98,20 @@ def test_ragged_shapes_long_sequences(api, w, p, heads, qscale):
     _check(api, 1, w, p, heads, oa.GLOBAL, 900 + s_len, scale=qscale, rows=rows, lse=True)
 
 
+@pytest.mark.parametrize("tail", [1, 31, 32, 33, 63, 64, 65, 96, 97, 127])
+def test_tail_tile_widths(api, tail):
+    # The ragged last KV tile is computed in 32-key chunks: only the chunks that hold keys are read and exponentiated, the
+    # P of the others is stored as zeros (attention.cu).  Every chunk boundary, on both head_dim 64 kernels: one, three and
+    # 65 KV tiles (the last on the one-item kernel, rows sampled), after a launch that leaves large values in TMEM.
+    big = synth.qkv(1, 1024, 2, 64, 5, device="cuda", scale=8.0)
+    api.window_attention(*big, 1, 1024, oa.GLOBAL)
+    for s_len in (tail, 256 + tail):
+        _check(api, 2, 1, s_len, 2, oa.GLOBAL, 31 * tail + s_len, lse=True)
+    s_len = 64 * 128 + tail
+    rows = np.unique(np.concatenate([np.arange(40), np.arange(s_len - 200, s_len)]))
+    _check(api, 1, 1, s_len, 1, oa.GLOBAL, 77 * tail, rows=rows, lse=True)
+
+
 def test_persistent_kernel_many_items_per_cta(api):
     # 148 SMs, 6000 work items of 2 KV tiles each: every CTA of the persistent kernel takes ~40 items through cluster launch
     # control; items with a dead second Q tile (S = 200 < 256... every item here) and live ones (S = 300) interleave per sequence
