@@ -84,7 +84,7 @@ __device__ __forceinline__ Item own_item() {
     it.qb = blockIdx.x; it.head = blockIdx.y; it.seq = blockIdx.z; it.valid = true;
     return it;
 }
-// Item number qi >= 1 of this CTA: wait for the response to the query the producer sent while item qi-1 began, decode it.
+// Item number qi >= 1 of this CTA (called by whole warps): wait for the response to the query the producer sent while item qi-1 began, decode it.
 // (Slot reuse: the query for item qi+4 is sent when the producer starts item qi+3, which needs the Q slot of item qi+1
 // released, i.e. every role well past reading the response for item qi.)
 __device__ __forceinline__ Item fetch_item(Smem& sm, int qi) {
@@ -100,8 +100,11 @@ __device__ __forceinline__ Item fetch_item(Smem& sm, int qi) {
         "@p1 clusterlaunchcontrol.query_cancel.get_first_ctaid.v4.b32.b128 {%0, %1, %2, _}, res;\n\t}"
         : "=r"(x), "=r"(y), "=r"(z), "=r"(valid) : "r"(ptx::smem_u32(sm.next_item[slot])) : "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");         // the slot is rewritten by the async proxy later
-    it.valid = valid != 0;
-    it.qb = static_cast<int>(x); it.head = static_cast<int>(y); it.seq = static_cast<int>(z);
+    // (every lane of the calling warp read the same 16 bytes; the shuffles tell the compiler so)
+    it.valid = __shfl_sync(0xffffffffu, valid, 0) != 0;
+    it.qb = static_cast<int>(__shfl_sync(0xffffffffu, x, 0));
+    it.head = static_cast<int>(__shfl_sync(0xffffffffu, y, 0));
+    it.seq = static_cast<int>(__shfl_sync(0xffffffffu, z, 0));
     return it;
 }
 // Ask the hardware for one more not-yet-started CTA of this grid; the 16-byte answer lands in next_item[slot].
@@ -118,7 +121,8 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                             const AttnParams prm) {
     extern __shared__ uint8_t smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (warp number through a shuffle: warp-uniform to the compiler, see attention.cu)
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
 
     if (warp == 8 && lane == 0) {
         ptx::prefetch_tensormap(&map_q);
@@ -171,38 +175,48 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         if (warp == 8) {
-            // ===================== TMA producer and work scheduler =====================
-            if (lane == 0) {
+            // ===================== TMA producer and work scheduler (whole warp in the loop, one elected lane issues) =====================
+            {
+                const bool leader = ptx::elect_one();
                 uint32_t kv = 0;                            // K/V tiles loaded so far (ring position)
                 Item it = own_item();
                 for (int qi = 0; it.valid; ++qi) {
-                    query_item(sm, qi + 1);                 // the item after this one, while this one is being loaded
+                    if (leader) query_item(sm, qi + 1);     // the item after this one, while this one is being loaded
                     const int slot = qi & 1, use = qi >> 1;
                     if (use > 0) ptx::mbar_wait(&sm.q_empty[slot], (use - 1) & 1);
-                    ptx::mbar_arrive_expect_tx(&sm.q_full[slot], kQTiles * kTileBytes);
-                    ptx::tma_load_4d(sm.q[slot][0], &map_q, &sm.q_full[slot], 0, it.head, it.row0(), it.seq);
                     // a dead second tile re-reads the first one (in bounds, never used); no output store will read its staging
                     // buffer, so the producer makes that arrival on the Q slot itself
                     const bool dead1 = !it.tile1_live(prm);
-                    ptx::tma_load_4d(sm.q[slot][1], &map_q, &sm.q_full[slot], 0, it.head, dead1 ? it.row0() : it.row0() + kBM, it.seq);
-                    if (dead1) ptx::mbar_arrive(&sm.q_empty[slot]);
+                    if (leader) {
+                        ptx::mbar_arrive_expect_tx(&sm.q_full[slot], kQTiles * kTileBytes);
+                        ptx::tma_load_4d(sm.q[slot][0], &map_q, &sm.q_full[slot], 0, it.head, it.row0(), it.seq);
+                        ptx::tma_load_4d(sm.q[slot][1], &map_q, &sm.q_full[slot], 0, it.head, dead1 ? it.row0() : it.row0() + kBM, it.seq);
+                        if (dead1) ptx::mbar_arrive(&sm.q_empty[slot]);
+                    }
                     for (int j = 0; j < n_kv; ++j, ++kv) {
                         const int st = kv % kStages;
                         const uint32_t ph = (kv / kStages) & 1;
                         ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
-                        ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
-                        ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, it.head, j * kBN, it.seq);
+                        if (leader) {
+                            ptx::mbar_arrive_expect_tx(&sm.k_full[st], kTileBytes);
+                            ptx::tma_load_4d(sm.k[st], &map_k, &sm.k_full[st], 0, it.head, j * kBN, it.seq);
+                        }
                         ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
-                        ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
-                        ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, it.head, j * kBN, it.seq);
-                                            }
+                        if (leader) {
+                            ptx::mbar_arrive_expect_tx(&sm.v_full[st], kTileBytes);
+                            ptx::tma_load_4d(sm.v[st], &map_v, &sm.v_full[st], 0, it.head, j * kBN, it.seq);
+                        }
+                    }
                     it = fetch_item(sm, qi + 1);
                 }
+                __syncwarp();
             }
         } else if (warp <= 10) {
             // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================
+            // (the whole warp runs the loop, one elected lane issues the MMAs, commits and arrives)
             const int t = warp - 9;
-            if (lane == 0) {
+            {
+                const bool leader = ptx::elect_one();
                 const uint32_t t_s = tmem + kColS + t * kBN, t_o = tmem + kColO + t * kON, t_p = tmem + kColP + t * kPH;
                 uint32_t kv = 0;                            // ring position of the tile whose P V comes next
                 uint32_t ns = 0;                            // S tiles issued so far (= phase counter of s_full / s_free)
@@ -214,9 +228,11 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                     if (ns > 0) ptx::mbar_wait(&sm.s_free[t], (ns - 1) & 1);      // the softmax warps hold the previous S in registers
                     ptx::mbar_wait(&sm.k_full[st], (kvi / kStages) & 1);
                     ptx::tc_fence_after();
-                    issue_qk(t_s, sm.q[slot][t], sm.k[st]);
-                    ptx::mma_commit(&sm.s_full[t]);
-                    ptx::mma_commit(&sm.k_empty[st]);
+                    if (leader) {
+                        issue_qk(t_s, sm.q[slot][t], sm.k[st]);
+                        ptx::mma_commit(&sm.s_full[t]);
+                        ptx::mma_commit(&sm.k_empty[st]);
+                    }
                     ++ns;
                 };
                 Item it = own_item();
@@ -230,14 +246,14 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         // for the one it is waiting for, and one that only watched, with the producer making its arrivals, could
                         // be lapped by the producer.  Both were tried; both deadlock on long runs of such items.)
                         ptx::mbar_wait(&sm.q_full[slot], (qi >> 1) & 1);
-                        ptx::mbar_arrive(&sm.q_empty[slot]);
+                        if (leader) ptx::mbar_arrive(&sm.q_empty[slot]);
                         for (int j = 0; j < n_kv; ++j, ++kv) {
                             const int st = kv % kStages;
                             const uint32_t ph = (kv / kStages) & 1;
                             ptx::mbar_wait(&sm.k_full[st], ph);
-                            ptx::mbar_arrive(&sm.k_empty[st]);
+                            if (leader) ptx::mbar_arrive(&sm.k_empty[st]);
                             ptx::mbar_wait(&sm.v_full[st], ph);
-                            ptx::mbar_arrive(&sm.v_empty[st]);
+                            if (leader) ptx::mbar_arrive(&sm.v_empty[st]);
                         }
                         have_s = false;
                         it = fetch_item(sm, qi + 1);
@@ -254,15 +270,16 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         if (j + 1 < n_kv) {
                             issue_s(slot, kv + 1);          // S(j+1) as soon as the softmax warpgroup holds S(j) in registers
                         } else {
-                            ptx::mma_commit(&sm.q_empty[slot]);             // every Q K^T of this item has been issued
+                            if (leader) ptx::mma_commit(&sm.q_empty[slot]);             // every Q K^T of this item has been issued
                             next = fetch_item(sm, qi + 1);  // (asked for when this item began: long since answered)
                             // The next item's S(0), ahead of this item's last P V -- but only if its Q tiles have landed: this
                             // thread must never BLOCK on the future while it still owes the present its P V.  (With one KV tile
                             // per item the next-but-one Q load waits for this item's output store, which waits for the softmax
                             // warps, which wait for this P V: a blocking wait here deadlocked S <= 128 launches of more than
                             // 148 items; found by differential fuzzing against attention.cu, ended by the watchdog.)
+                            // (one decision for the warp: all lanes must have seen the phase complete)
                             if (next.valid && (t == 0 || next.tile1_live(prm)) &&
-                                ptx::mbar_try_wait(&sm.q_full[slot ^ 1], ((qi + 1) >> 1) & 1)) {
+                                __all_sync(0xffffffffu, ptx::mbar_try_wait(&sm.q_full[slot ^ 1], ((qi + 1) >> 1) & 1))) {
                                 issue_s(slot ^ 1, kv + 1);
                                 have_s = true;
                             }
@@ -274,14 +291,17 @@ window_attention_clc_kernel(const __grid_constant__ CUtensorMap map_q, const __g
                         for (int h = 0; h < 2; ++h) {
                             ptx::mbar_wait(&sm.p_full[h][t], np & 1);
                             ptx::tc_fence_after();
-                            issue_pv_half(t_o, t_p, sm.v[st] + h * (kTileBytes / 2), ones_minus_v, j > 0 || h > 0);
-                            ptx::mma_commit(&sm.pv_done[h][t]);
+                            if (leader) {
+                                issue_pv_half(t_o, t_p, sm.v[st] + h * (kTileBytes / 2), ones_minus_v, j > 0 || h > 0);
+                                ptx::mma_commit(&sm.pv_done[h][t]);
+                            }
                         }
-                        ptx::mma_commit(&sm.v_empty[st]);
+                        if (leader) ptx::mma_commit(&sm.v_empty[st]);
                     }
                     ++live_items;
                     it = next;
                 }
+                __syncwarp();
             }
         } else if (lane == 0) {
             ptx::watchdog_progress(&sm.roles_done, sm.k_full);                // warp 11: traps if the 11 role warps do not finish within seconds

@@ -81,7 +81,8 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                              const __grid_constant__ CUtensorMap map_v, const AttnParams prm) {
     extern __shared__ uint8_t smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (warp number through a shuffle: warp-uniform to the compiler, see attention.cu)
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
 
     const int qb = blockIdx.x % prm.q_blocks;
     const int head = (blockIdx.x / prm.q_blocks) % prm.heads;
@@ -125,41 +126,50 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tmem = sm.tmem_base;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, sm.tmem_base, 0);       // (uniform, as above)
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         if (warp == 8) {
-            // ===================== TMA producer =====================
-            if (lane == 0) {
+            // ===================== TMA producer (whole warp in the loop, one elected lane issues) =====================
+            const bool leader = ptx::elect_one();
+            if (leader) {
                 ptx::mbar_arrive_expect_tx(&sm.q_full, (tile1_live ? 4 : 2) * kQHalfBytes);
                 for (int t = 0; t < (tile1_live ? 2 : 1); ++t)
                     for (int h = 0; h < 2; ++h)
                         ptx::tma_load_4d(sm.q[t][h], &map_q, &sm.q_full, h * kDH, head, row0 + t * kBM, seq);
-                for (int j = 0; j < n_kv; ++j) {
-                    const int st = j % kStages;
-                    const uint32_t ph = (j / kStages) & 1;
-                    ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
+            }
+            for (int j = 0; j < n_kv; ++j) {
+                const int st = j % kStages;
+                const uint32_t ph = (j / kStages) & 1;
+                ptx::mbar_wait(&sm.k_empty[st], ph ^ 1);
+                if (leader) {
                     ptx::mbar_arrive_expect_tx(&sm.k_full[st], 2 * kKVHalfBytes);
                     ptx::tma_load_4d(sm.k[st][0], &map_k, &sm.k_full[st], 0, head, j * kBN, seq);
                     ptx::tma_load_4d(sm.k[st][1], &map_k, &sm.k_full[st], kDH, head, j * kBN, seq);
-                    ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
+                }
+                ptx::mbar_wait(&sm.v_empty[st], ph ^ 1);
+                if (leader) {
                     ptx::mbar_arrive_expect_tx(&sm.v_full[st], 2 * kKVHalfBytes);
                     ptx::tma_load_4d(sm.v[st].lo, &map_v, &sm.v_full[st], 0, head, j * kBN, seq);
                     ptx::tma_load_4d(sm.v[st].hi, &map_v, &sm.v_full[st], kDH, head, j * kBN, seq);
-                                    }
+                }
             }
+            __syncwarp();
         } else if (warp <= 10) {
-            // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1) =====================
+            // ===================== MMA issuers (warp 9: Q tile 0, warp 10: Q tile 1; one elected lane issues) =====================
             const int t = warp - 9;
-            if (lane == 0 && (t == 0 || tile1_live)) {
+            if (t == 0 || tile1_live) {
+                const bool leader = ptx::elect_one();
                 const uint32_t t_s = tmem + kColS + t * kBN, t_o = tmem + kColO + t * kON, t_p = tmem + kColP + t * kPCols;
                 ptx::mbar_wait(&sm.q_full, 0);
                 ptx::mbar_wait(&sm.k_full[0], 0);
                 ptx::tc_fence_after();
-                issue_qk(t_s, sm.q[t], sm.k[0]);
-                ptx::mma_commit(&sm.s_full[t]);
-                ptx::mma_commit(&sm.k_empty[0]);
+                if (leader) {
+                    issue_qk(t_s, sm.q[t], sm.k[0]);
+                    ptx::mma_commit(&sm.s_full[t]);
+                    ptx::mma_commit(&sm.k_empty[0]);
+                }
                 for (int j = 0; j < n_kv; ++j) {
                     const int st = j % kStages;
                     if (j + 1 < n_kv) {
@@ -168,17 +178,22 @@ window_attention_d128_kernel(const __grid_constant__ CUtensorMap map_q, const __
                         ptx::mbar_wait(&sm.s_free[t], j & 1);
                         ptx::mbar_wait(&sm.k_full[st1], ((j + 1) / kStages) & 1);
                         ptx::tc_fence_after();
-                        issue_qk(t_s, sm.q[t], sm.k[st1]);
-                        ptx::mma_commit(&sm.s_full[t]);
-                        ptx::mma_commit(&sm.k_empty[st1]);
+                        if (leader) {
+                            issue_qk(t_s, sm.q[t], sm.k[st1]);
+                            ptx::mma_commit(&sm.s_full[t]);
+                            ptx::mma_commit(&sm.k_empty[st1]);
+                        }
                     }
                     ptx::mbar_wait(&sm.v_full[st], (j / kStages) & 1);
                     ptx::mbar_wait(&sm.p_full[t], j & 1);
                     ptx::tc_fence_after();
-                    issue_pv(t_o, t_p, sm.v[st], j > 0);
-                    ptx::mma_commit(&sm.pv_done[t]);
-                    ptx::mma_commit(&sm.v_empty[st]);
+                    if (leader) {
+                        issue_pv(t_o, t_p, sm.v[st], j > 0);
+                        ptx::mma_commit(&sm.pv_done[t]);
+                        ptx::mma_commit(&sm.v_empty[st]);
+                    }
                 }
+                __syncwarp();
             }
         } else if (lane == 0) {
             ptx::watchdog(&sm.roles_done);            // warp 11: traps if the 11 role warps do not finish within seconds
