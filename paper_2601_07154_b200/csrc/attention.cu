@@ -26,6 +26,7 @@
 
 #include <cuda_bf16.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cstddef>
 #include <mutex>
@@ -44,7 +45,8 @@ constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kColS = 0, kColO = 256, kColP = 416;
 constexpr int kON = 80;                // PV accumulator columns: 64 outputs + column 64 = row sum l (+15 unused)
 constexpr int kPH = 32;                // TMEM columns of one P half (64 keys, bf16)
-constexpr float kRescaleThreshold = 8.0f;          // log2 units
+constexpr float kRescaleThreshold = 8.0f;
+constexpr float kScoreBoundMax = 32.0f;    // log2 units: the score-bound path is taken for rows with |q| max|k| scale log2(e) <= 32 (22 nats)          // log2 units
 #ifndef MF_POLY_PAIRS
 #define MF_POLY_PAIRS 4                // of every 16 score pairs, this many are exponentiated on the FMA pipe
 #endif
@@ -250,7 +252,8 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
             // quarter of the softmax work of a full tile; FRAME mode +5.5 %).  The MMA issuers do not know about it: narrowing
             // the tail's Q K^T and P V too was measured, and the extra selects and predicates in the issuing thread cost the
             // steady state 2 % (campus) to 4 % (suburban), for no gain on the tail.
-            auto kv_tile = [&](const int j, auto tail) {
+            auto kv_tile = [&](const int j, auto tail, auto bounded_tag) {
+                constexpr bool kBounded = decltype(bounded_tag)::value;          // m_used is the row's score bound: no maximum, no rescaling
                 constexpr bool kMasked = decltype(tail)::value != 0;
                 constexpr int kChunks = kMasked ? decltype(tail)::value : 4;
                 ptx::mbar_wait(a_s_full, j & 1);
@@ -278,38 +281,40 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     // adds at most 2^-125 per key to the row sum l >= 1.  Zeroing those words exactly was measured: a
                     // uniform branch with 96 selects on every tail tile costs 6 % in FRAME mode, for no change in O.)
                 }
-                float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+                if (!kBounded) {
+                    float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-                for (int c = 0; c < kChunks; ++c)
+                    for (int c = 0; c < kChunks; ++c)
 #pragma unroll
-                    for (int i = 0; i < 32; i += 8)
+                        for (int i = 0; i < 32; i += 8)
 #pragma unroll
-                        for (int a = 0; a < 4; ++a)
-                            mx[a] = ptx::max3(mx[a], __uint_as_float(s[c][i + 2 * a]), __uint_as_float(s[c][i + 2 * a + 1]));
-                const float row_max = ptx::max3(fmaxf(mx[0], mx[1]), mx[2], mx[3]);
-                const float m_new = fmaxf(m_used, row_max * prm.scale_log2);
-                const bool grow = m_new > m_used + kRescaleThreshold;            // always true at j == 0
-                if (j == 0) {
-                    m_used = m_new;
-                } else if (__any_sync(0xffffffffu, grow)) {
-                    // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
-                    ptx::mbar_wait(a_pv_done1, (j - 1) & 1);
-                    ptx::tc_fence_after();
-                    const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
-                    if (grow) m_used = m_new;
-                    const uint64_t alpha2 = ptx::pack2(alpha, alpha);
+                            for (int a = 0; a < 4; ++a)
+                                mx[a] = ptx::max3(mx[a], __uint_as_float(s[c][i + 2 * a]), __uint_as_float(s[c][i + 2 * a + 1]));
+                    const float row_max = ptx::max3(fmaxf(mx[0], mx[1]), mx[2], mx[3]);
+                    const float m_new = fmaxf(m_used, row_max * prm.scale_log2);
+                    const bool grow = m_new > m_used + kRescaleThreshold;            // always true at j == 0
+                    if (j == 0) {
+                        m_used = m_new;
+                    } else if (__any_sync(0xffffffffu, grow)) {
+                        // O may only be touched once PV(j-1) has completed; PV(j) is not issued before p_full(j)
+                        ptx::mbar_wait(a_pv_done1, (j - 1) & 1);
+                        ptx::tc_fence_after();
+                        const float alpha = grow ? ptx::ex2(m_used - m_new) : 1.0f;
+                        if (grow) m_used = m_new;
+                        const uint64_t alpha2 = ptx::pack2(alpha, alpha);
 #pragma unroll
-                    for (int c = 0; c < 2; ++c) {
-                        uint32_t o[32];
-                        ptx::tmem_ld32(t_o + 32 * c, o);
+                        for (int c = 0; c < 2; ++c) {
+                            uint32_t o[32];
+                            ptx::tmem_ld32(t_o + 32 * c, o);
+                            ptx::tc_wait_ld();
+#pragma unroll
+                            for (int i = 0; i < 32; i += 2) ptx::fmul2(o[i], o[i + 1], alpha2);
+                            ptx::tmem_st32(t_o + 32 * c, o);
+                        }
+                        const float l_old = __uint_as_float(ptx::tmem_ld1(t_o + kD));
                         ptx::tc_wait_ld();
-#pragma unroll
-                        for (int i = 0; i < 32; i += 2) ptx::fmul2(o[i], o[i + 1], alpha2);
-                        ptx::tmem_st32(t_o + 32 * c, o);
+                        ptx::tmem_st1(t_o + kD, __float_as_uint(l_old * alpha));
                     }
-                    const float l_old = __uint_as_float(ptx::tmem_ld1(t_o + kD));
-                    ptx::tc_wait_ld();
-                    ptx::tmem_st1(t_o + kD, __float_as_uint(l_old * alpha));
                 }
                 const uint64_t neg_m2 = ptx::pack2(-m_used, -m_used);
                 uint64_t scale_h = scale2;
@@ -353,12 +358,43 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     }
                 }
             };
-            for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::integral_constant<int, 0>{});
-            const int tail_chunks = (prm.seq_len - (n_kv - 1) * kBN + 31) / 32;        // 1..4
-            if (prm.seq_len % kBN == 0) kv_tile(n_kv - 1, std::integral_constant<int, 0>{});
-            else if (tail_chunks == 1) kv_tile(n_kv - 1, std::integral_constant<int, 1>{});
-            else if (tail_chunks == 2) kv_tile(n_kv - 1, std::integral_constant<int, 2>{});
-            else kv_tile(n_kv - 1, std::integral_constant<int, 4>{});
+            auto all_tiles = [&](auto bounded_tag) {
+                for (int j = 0; j + 1 < n_kv; ++j) kv_tile(j, std::integral_constant<int, 0>{}, bounded_tag);
+                const int tail_chunks = (prm.seq_len - (n_kv - 1) * kBN + 31) / 32;        // 1..4
+                if (prm.seq_len % kBN == 0) kv_tile(n_kv - 1, std::integral_constant<int, 0>{}, bounded_tag);
+                else if (tail_chunks == 1) kv_tile(n_kv - 1, std::integral_constant<int, 1>{}, bounded_tag);
+                else if (tail_chunks == 2) kv_tile(n_kv - 1, std::integral_constant<int, 2>{}, bounded_tag);
+                else kv_tile(n_kv - 1, std::integral_constant<int, 4>{}, bounded_tag);
+            };
+            // Score bound (Cauchy-Schwarz): every score of row i is at most |q_i| max_j |k_j|.  Softmax is invariant under the
+            // choice of the subtracted constant, so when that bound is small enough that 2^(score - bound) stays far inside
+            // the range of bf16 / fp32 (bound <= kScoreBoundMax: the largest weight of the row is then >= 2^-2*kScoreBoundMax),
+            // the bound itself serves as the row's "maximum": no maximum over the scores, no rescaling of O, and nothing that an
+            // exponential has to wait for (campus launch: +7.8 %).  The key norms come from a pass over K before this kernel
+            // (key_norm_max_kernel); |q_i|^2 is summed from the row's 128 bytes in shared memory.  The decision is taken per
+            // warp; rows with a larger bound (peaked logits), NaN or Inf anywhere in it take the exact online-softmax path.
+            bool bounded = false;
+            if (prm.key_norm2_max != nullptr) {
+                ptx::mbar_wait(sb + offsetof(AttnSmem, q_full), 0);
+                const uint4* q_row = reinterpret_cast<const uint4*>(sm.q[tile] + row_in_tile * (kD * 2));
+                float qq = 0.f;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {             // (the swizzle permutes the row's eight 16-byte chunks: irrelevant to a sum)
+                    const uint4 w = q_row[(c + lane) & 7];
+                    const uint32_t u[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const float lo = __uint_as_float(u[i] << 16), hi = __uint_as_float(u[i] & 0xffff0000u);
+                        qq = fmaf(lo, lo, fmaf(hi, hi, qq));
+                    }
+                }
+                const float kk = prm.key_norm2_max[static_cast<size_t>(seq) * prm.heads + head];
+                const float bound = sqrtf(qq * kk) * fabsf(prm.scale_log2) * (1.0f + 0x1p-10f);       // (slack: fp32 rounding of the sums and of S)
+                bounded = __all_sync(0xffffffffu, bound <= kScoreBoundMax);
+                if (bounded) m_used = bound;
+            }
+            if (bounded) all_tiles(std::true_type{});
+            else all_tiles(std::false_type{});
             // ---- epilogue: O / l -> bf16 -> global ----
             ptx::mbar_wait(a_pv_done1, (n_kv - 1) & 1);
             ptx::tc_fence_after();
@@ -402,6 +438,47 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 9) ptx::tmem_dealloc(tmem, kTmemCols);
+}
+
+// Pass over K before window_attention_kernel: out[sequence, head] = max over the tokens of |k|^2, as float bits (non-negative
+// floats order like unsigned integers, so the maximum is an atomicMax and does not depend on the order of arrival; a NaN
+// anywhere has the largest bits and survives: the attention kernel then takes its exact path).  K is [sequences, S, H, 64]
+// bf16: a (token, head) row is eight 16-byte chunks, summed by eight neighbouring lanes.  HBM-bound: K is read once.
+__global__ void __launch_bounds__(256)
+key_norm_max_kernel(const uint4* __restrict__ k, uint32_t* __restrict__ out, long long rows_per_sequence, int heads) {
+    extern __shared__ uint32_t head_max[];                 // [heads]
+    for (int i = threadIdx.x; i < heads; i += blockDim.x) head_max[i] = 0u;
+    __syncthreads();
+    const uint4* base = k + static_cast<size_t>(blockIdx.y) * rows_per_sequence * 8;
+    const long long chunks = rows_per_sequence * 8;         // (token, head) rows x 8
+    const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+    constexpr int kUnroll = 4;
+    for (long long g0 = static_cast<long long>(blockIdx.x) * blockDim.x + (threadIdx.x & ~31); g0 < chunks; g0 += kUnroll * stride) {
+        uint4 w[kUnroll];
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+            const long long g = g0 + u * stride + (threadIdx.x & 31);
+            w[u] = g < chunks ? __ldg(base + g) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+            const long long g = g0 + u * stride + (threadIdx.x & 31);
+            const uint32_t x[4] = {w[u].x, w[u].y, w[u].z, w[u].w};
+            float ss = 0.f;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float lo = __uint_as_float(x[i] << 16), hi = __uint_as_float(x[i] & 0xffff0000u);
+                ss = fmaf(lo, lo, fmaf(hi, hi, ss));
+            }
+            ss += __shfl_xor_sync(0xffffffffu, ss, 1);
+            ss += __shfl_xor_sync(0xffffffffu, ss, 2);
+            ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+            if ((threadIdx.x & 7) == 0 && g < chunks) atomicMax(&head_max[(g >> 3) % heads], __float_as_uint(ss));
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < heads; i += blockDim.x)
+        if (head_max[i] != 0u) atomicMax(&out[static_cast<size_t>(blockIdx.y) * heads + i], head_max[i]);
 }
 
 }  // namespace mf
@@ -461,6 +538,36 @@ static mf_status cached_map(CUtensorMap* out, const void* base, int sequences, i
     return MF_OK;
 }
 
+// Stream-ordered workspace for the score bound ([sequences, heads] floats): allocated and freed on the caller's stream from a
+// pool of the library's own (cudaMallocFromPoolAsync: no synchronisation, safe with concurrent callers on other streams and
+// inside stream capture, where it becomes a pair of graph nodes).  The pool keeps its memory between calls.
+static mf_status bound_workspace(uint32_t** p, size_t bytes, cudaStream_t stream) {
+    static std::mutex mu;
+    static cudaMemPool_t pools[64];
+    static bool made[64];
+    int dev = 0;
+    MF_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(MF_ERR_UNSUPPORTED, "device ordinal %d", dev);
+    cudaMemPool_t pool;
+    {
+        std::lock_guard<std::mutex> g(mu);
+        if (!made[dev]) {
+            cudaMemPoolProps props = {};
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = dev;
+            MF_CUDA_OK(cudaMemPoolCreate(&pools[dev], &props));
+            uint64_t keep = ~0ull;
+            MF_CUDA_OK(cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep));
+            made[dev] = true;
+        }
+        pool = pools[dev];
+    }
+    MF_CUDA_OK(cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes, pool, stream));
+    return MF_OK;
+}
+
 }  // namespace mf
 
 extern "C" mf_status mf_window_attention(const void* q, const void* k, const void* v, void* out, float* lse,
@@ -490,9 +597,6 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if (static_cast<long long>((seq_len + 255) / 256) * heads * sequences > 0x7fffffffLL)
         return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
     if (validate_only()) return MF_OK;
-    if (static_cast<long long>((seq_len + 255) / 256) * heads * sequences > 0x7fffffffLL)
-        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention: grid too large");
-    if (validate_only()) return MF_OK;
 
     AttnParams prm;
     prm.seq_len = seq_len;
@@ -503,6 +607,7 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     prm.out = static_cast<__nv_bfloat16*>(out);
     prm.lse = lse;
     prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
+    prm.key_norm2_max = nullptr;
     if (head_dim == 128)       // re-tiled variant (attention_d128.cu); q_blocks is the same: 256 query rows per CTA
         return launch_attention_d128(q, k, v, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
 
@@ -525,7 +630,26 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
             if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
         }
     }
-    window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(mq, mk, mv, prm);
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    uint32_t* bound_ws = nullptr;
+#ifndef MF_NO_SCORE_BOUND          // (test builds: tests/test_gpu_attention_differential.py compares the exact paths of the two kernels bit for bit)
+    if (heads <= 4096 && sequences <= 65535) {
+        // the score bound's pass over K (window_attention_kernel: "Score bound"); 0.3 % of the attention launch at S = 24864
+        const size_t ws_bytes = static_cast<size_t>(sequences) * heads * sizeof(uint32_t);
+        if ((st = bound_workspace(&bound_ws, ws_bytes, cs)) != MF_OK) return st;
+        MF_CUDA_OK(cudaMemsetAsync(bound_ws, 0, ws_bytes, cs));
+        const long long rows = static_cast<long long>(seq_len) * heads;
+        const long long want = (rows * 8 + 256 * 4 - 1) / (256 * 4);
+        const long long cap = (8LL * sm_count() + sequences - 1) / sequences;
+        const unsigned gx = static_cast<unsigned>(std::max(1LL, std::min(want, cap)));
+        key_norm_max_kernel<<<dim3(gx, static_cast<unsigned>(sequences)), 256, heads * sizeof(uint32_t), cs>>>(
+            static_cast<const uint4*>(k), bound_ws, rows, heads);
+        MF_CUDA_OK(cudaGetLastError());
+        prm.key_norm2_max = reinterpret_cast<const float*>(bound_ws);
+    }
+#endif
+    window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, cs>>>(mq, mk, mv, prm);
     MF_CUDA_OK(cudaGetLastError());
+    if (bound_ws) MF_CUDA_OK(cudaFreeAsync(bound_ws, cs));
     return MF_OK;
 }

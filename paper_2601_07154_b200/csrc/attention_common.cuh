@@ -15,6 +15,7 @@ struct AttnParams {
     __nv_bfloat16* out;
     float* lse;         // [windows, heads, S] or nullptr
     int lse_frames;     // sequences per window (W in frame mode, 1 in global mode)
+    const float* key_norm2_max;   // [sequences, heads] max over the keys of |k|^2 (attention.cu: the score bound), or nullptr
 };
 
 // (2^x0, 2^x1) on the FMA pipe.  x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a cubic (minimax in

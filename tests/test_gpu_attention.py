@@ -112,6 +112,57 @@ def test_tail_tile_widths(api, tail):
     _check(api, 1, 1, s_len, 1, oa.GLOBAL, 77 * tail, rows=rows, lse=True)
 
 
+def _long_rows(s_len, seed):
+    rng = np.random.default_rng(seed)
+    return np.unique(np.concatenate([np.arange(64), np.arange(s_len - 200, s_len), rng.integers(0, s_len, 128)]))
+
+
+def _compare(api, q, k, v, s_len, rows, lse_bar=4e-3):
+    out, lse = api.window_attention(q, k, v, 1, s_len, oa.GLOBAL, return_lse=True)
+    torch.cuda.synchronize()
+    ref, lse_ref = oa.window_attention(_to64(q), _to64(k), _to64(v), 1, s_len, oa.GLOBAL, rows=rows)
+    got = _to64(out)[:, rows]
+    assert np.isfinite(got).all()
+    for n in range(q.shape[0]):
+        d = got[n] - ref[n]
+        assert np.abs(d).max() <= MAX_ABS and np.linalg.norm(d) / np.linalg.norm(ref[n]) <= REL_L2
+        _per_row(d, ref[n], ("score bound", n))
+    assert np.abs(lse.cpu().numpy().astype(np.float64)[:, :, rows] - lse_ref).max() <= lse_bar
+
+
+def test_score_bound_mixed_rows(api):
+    # Long sequences (one-item kernel) subtract the row's Cauchy-Schwarz bound |q_i| max|k| instead of the running maximum when
+    # it is <= 32 log2 units, decided per warp (attention.cu).  Query rows scaled x1 / x3 / x8 in blocks of 32 and of 7 rows:
+    # warps on the bound path, warps on the exact path and warps that hold both kinds of row, in one launch.
+    s_len = 64 * 128 + 40
+    q, k, v = synth.qkv(1, s_len, 2, 64, 2024, device="cuda")
+    f = torch.ones(s_len, device="cuda")
+    f[32:64] = 3.0
+    f[64:96] = 8.0
+    f[200:207] = 8.0
+    f[s_len - 100:s_len - 60] = 3.0
+    f[s_len - 30:] = 8.0
+    q = (q.float() * f[None, :, None, None]).to(torch.bfloat16)
+    _compare(api, q, k, v, s_len, _long_rows(s_len, 1))
+
+
+def test_score_bound_far_above_the_scores(api):
+    # The bound is tight only when q is aligned with the longest key.  Worst case for it: every key equal to u and q = -t u,
+    # so all scores sit at MINUS the bound and the weights are 2^(-2 bound) before normalisation (t chosen so the bound is
+    # ~30 log2 units: just inside the path's guard): the result must still be the plain mean of V.
+    s_len = 64 * 128 + 5
+    u = torch.randn(64, device="cuda")
+    u = u / u.norm() * 8.0
+    k = u.to(torch.bfloat16)[None, None, None, :].expand(1, s_len, 1, 64).contiguous()
+    q = (-2.55 * u).to(torch.bfloat16)[None, None, None, :].expand(1, s_len, 1, 64).contiguous()      # |q||k|/8 = 20.4 nats = 29.4 log2 units
+    v = synth.qkv(1, s_len, 1, 64, 7, device="cuda")[2]
+    _compare(api, q, k, v, s_len, _long_rows(s_len, 2))
+    # and one very long key among ordinary ones: the bound leaves the guard, every row takes the exact path
+    q2, k2, v2 = synth.qkv(1, s_len, 1, 64, 8, device="cuda")
+    k2[0, 4321] *= 40.0
+    _compare(api, q2, k2, v2, s_len, _long_rows(s_len, 3))
+
+
 def test_persistent_kernel_many_items_per_cta(api):
     # 148 SMs, 6000 work items of 2 KV tiles each: every CTA of the persistent kernel takes ~40 items through cluster launch
     # control; items with a dead second Q tile (S = 200 < 256... every item here) and live ones (S = 300) interleave per sequence

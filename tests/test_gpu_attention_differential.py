@@ -1,7 +1,8 @@
 """Differential test of the two head_dim 64 attention kernels.  Sequences below 64 KV tiles run on the persistent kernel
 (attention_clc.cu: work items handed out by cluster launch control, many items per CTA), longer ones on the one-item-per-CTA
 kernel (attention.cu).  Both run the same tile pipeline in the same order, so on the same inputs their outputs must be
-BIT-IDENTICAL.  A second build of the library with the persistent kernel switched off (-DMF_PERSISTENT_BELOW_TILES=0) supplies
+BIT-IDENTICAL.  A second build of the library with the persistent kernel switched off (-DMF_PERSISTENT_BELOW_TILES=0; and
+-DMF_NO_SCORE_BOUND, so that the one-item kernel takes its exact online-softmax path like the persistent one) supplies
 the other side; seeded random shapes put many items on every CTA, with one to sixty KV tiles per item and live / dead second
 Q tiles in every order.  (This is how the two deadlocks of the persistent kernel's protocol were found: DESIGN.md 6.1.)
 The oracle comparison of both kernels is tests/test_gpu_attention.py; this test is about the pipeline protocol."""
@@ -24,7 +25,7 @@ def libs(tmp_path_factory):
     sys.path.insert(0, root)
     from paper_2601_07154_b200 import api, build
     tmp = tmp_path_factory.mktemp("nopersist")
-    other = build.build(out=str(tmp / "libmf_nopersist.so"), extra_flags=["-DMF_PERSISTENT_BELOW_TILES=0"], build_dir=str(tmp / "obj"))
+    other = build.build(out=str(tmp / "libmf_nopersist.so"), extra_flags=["-DMF_PERSISTENT_BELOW_TILES=0", "-DMF_NO_SCORE_BOUND"], build_dir=str(tmp / "obj"))
     new = api.lib()
     old = ctypes.CDLL(other)
     old.mf_window_attention.argtypes = new.mf_window_attention.argtypes
