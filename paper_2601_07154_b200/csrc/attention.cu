@@ -46,13 +46,12 @@ constexpr uint32_t kColS = 0, kColO = 256, kColP = 416;
 constexpr int kON = 80;                // PV accumulator columns: 64 outputs + column 64 = row sum l (+15 unused)
 constexpr int kPH = 32;                // TMEM columns of one P half (64 keys, bf16)
 constexpr float kRescaleThreshold = 8.0f;
-constexpr float kScoreBoundMax = 32.0f;    // log2 units: the score-bound path is taken for rows with |q| max|k| scale log2(e) <= 32 (22 nats)          // log2 units
-#ifndef MF_POLY_PAIRS
-#define MF_POLY_PAIRS 4                // of every 16 score pairs, this many are exponentiated on the FMA pipe
+constexpr float kScoreBoundMax = 32.0f;    // log2 units: the score-bound path is taken for rows with |q| max|k| scale log2(e) <= 32 (22 nats)
+#ifndef MF_POLY_PAIRS_BOUND
+#define MF_POLY_PAIRS_BOUND 6          // the same on the score-bound path, which has issue slots to spare (5: -0.6 %, 7: -2.3 %)
 #endif
-constexpr int kPolyPairs = MF_POLY_PAIRS;
 #ifndef MF_PERSISTENT_BELOW_TILES
-#define MF_PERSISTENT_BELOW_TILES 64   // sequences of fewer KV tiles (S <= 8064) run on the persistent kernel (attention_clc.cu)
+#define MF_PERSISTENT_BELOW_TILES 32   // sequences of fewer KV tiles (S <= 3968) run on the persistent kernel (attention_clc.cu); with the score-bound path here, S = 6216 gains 4 % on this kernel, S = 1024 loses 19 %
 #endif
 constexpr int kPersistentBelowTiles = MF_PERSISTENT_BELOW_TILES;
 
@@ -325,6 +324,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
                             ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
+                            constexpr int kPolyPairs = kBounded ? MF_POLY_PAIRS_BOUND : MF_POLY_PAIRS;
                             if (((((i >> 1) & 15) * kPolyPairs) & 15) < kPolyPairs) {       // kPolyPairs of every 16 pairs, evenly spread
                                 exp2_poly2(s[c][i], s[c][i + 1]);
                             } else {
@@ -541,6 +541,7 @@ static mf_status cached_map(CUtensorMap* out, const void* base, int sequences, i
 // Stream-ordered workspace for the score bound ([sequences, heads] floats): allocated and freed on the caller's stream from a
 // pool of the library's own (cudaMallocFromPoolAsync: no synchronisation, safe with concurrent callers on other streams and
 // inside stream capture, where it becomes a pair of graph nodes).  The pool keeps its memory between calls.
+#ifndef MF_NO_SCORE_BOUND
 static mf_status bound_workspace(uint32_t** p, size_t bytes, cudaStream_t stream) {
     static std::mutex mu;
     static cudaMemPool_t pools[64];
@@ -567,6 +568,7 @@ static mf_status bound_workspace(uint32_t** p, size_t bytes, cudaStream_t stream
     MF_CUDA_OK(cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes, pool, stream));
     return MF_OK;
 }
+#endif
 
 }  // namespace mf
 

@@ -1,4 +1,4 @@
-// mf_window_attention, head_dim 64, short sequences (fewer than 64 KV tiles: FRAME mode, S <= 8064): the same tile pipeline as
+// mf_window_attention, head_dim 64, short sequences (fewer than 32 KV tiles: FRAME mode, S <= 3968): the same tile pipeline as
 // window_attention_kernel (attention.cu), made PERSISTENT with Blackwell's cluster launch control.
 //
 // A CTA of attention.cu lives for one work item (sequence, head, 256 query rows).  With 7 KV tiles per item (P = 777) its
@@ -38,7 +38,7 @@ constexpr uint32_t kColS = 0, kColO = 256, kColP = 416;
 constexpr int kON = 80;                // PV accumulator columns: 64 outputs + column 64 = row sum l (+15 unused)
 constexpr int kPH = 32;                // TMEM columns of one P half (64 keys, bf16)
 constexpr float kRescaleThreshold = 8.0f;
-constexpr int kPolyPairs = 4;          // of every 16 score pairs, this many are exponentiated on the FMA pipe
+constexpr int kPolyPairs = MF_POLY_PAIRS;          // (attention_common.cuh)
 
 struct Smem {
     alignas(1024) uint8_t q[kQSlots][kQTiles][kTileBytes];

@@ -5,6 +5,12 @@
 
 #include <cuda_bf16.h>
 
+// Of every 16 score pairs, this many are exponentiated on the FMA pipe instead of the MUFU (the two head_dim 64 kernels share
+// the value: their exact paths are compared bit for bit, tests/test_gpu_attention_differential.py).
+#ifndef MF_POLY_PAIRS
+#define MF_POLY_PAIRS 5
+#endif
+
 namespace mf {
 
 struct AttnParams {

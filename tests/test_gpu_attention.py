@@ -90,7 +90,7 @@ def test_ragged_shapes(api, windows, w, p, heads, mode):
     (1, 8321, 1, 1.0),       # one key into the 66th tile
 ])
 def test_ragged_shapes_long_sequences(api, w, p, heads, qscale):
-    # Sequences of 64 KV tiles and more run on the one-item-per-CTA kernel (attention.cu), shorter ones on the persistent
+    # Sequences of 32 KV tiles and more run on the one-item-per-CTA kernel (attention.cu), shorter ones on the persistent
     # kernel (attention_clc.cu): the ragged cases above the switch, GLOBAL mode, oracle on sampled rows (reading A7)
     s_len = w * p
     rng = np.random.default_rng(s_len)

@@ -1,9 +1,9 @@
-"""Differential test of the two head_dim 64 attention kernels.  Sequences below 64 KV tiles run on the persistent kernel
+"""Differential test of the two head_dim 64 attention kernels.  Sequences below 32 KV tiles run on the persistent kernel
 (attention_clc.cu: work items handed out by cluster launch control, many items per CTA), longer ones on the one-item-per-CTA
 kernel (attention.cu).  Both run the same tile pipeline in the same order, so on the same inputs their outputs must be
 BIT-IDENTICAL.  A second build of the library with the persistent kernel switched off (-DMF_PERSISTENT_BELOW_TILES=0; and
 -DMF_NO_SCORE_BOUND, so that the one-item kernel takes its exact online-softmax path like the persistent one) supplies
-the other side; seeded random shapes put many items on every CTA, with one to sixty KV tiles per item and live / dead second
+the other side; seeded random shapes put many items on every CTA, with one to thirty-one KV tiles per item and live / dead second
 Q tiles in every order.  (This is how the two deadlocks of the persistent kernel's protocol were found: DESIGN.md 6.1.)
 The oracle comparison of both kernels is tests/test_gpu_attention.py; this test is about the pipeline protocol."""
 import ctypes
@@ -49,8 +49,8 @@ def test_persistent_kernel_equals_one_item_kernel_bit_for_bit(libs, seed):
     for _ in range(60):
         w, p = int(rng.integers(1, 6)), int(rng.integers(1, 700))
         heads, windows, mode = int(rng.integers(1, 21)), int(rng.integers(1, 120)), int(rng.integers(0, 2))
-        if mode == 0 and w * p > 8000:
-            p = 8000 // w
+        if mode == 0 and w * p > 3900:          # (32 KV tiles and more never reach the persistent kernel)
+            p = 3900 // w
         case = dict(windows=windows, w=w, p=p, heads=heads, mode=mode)
         q, k, v = synth.qkv(windows, w * p, heads, 64, int(rng.integers(0, 1 << 30)), device="cuda", scale=float(rng.choice([1.0, 2.0, 6.0])))
         a, la = _run(new, q, k, v, windows, w, p, heads, mode)
