@@ -200,6 +200,22 @@ mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intrinsics K, i
                                     float* focus_uv, int32_t* focus_index, void* workspace,
                                     size_t workspace_bytes, void* stream);
 
+/* mf_window_attention for callers that cannot allocate device memory (CUDA graph capture, serving loops, harnesses that
+ * forbid it).  Same arguments, semantics, checks and results as mf_window_attention.  The one scratch buffer that call
+ * takes from a stream-ordered pool (head_dim 64, sequences of 32 KV tiles and more: [sequences, heads] floats holding
+ * max |k|^2 for the score bound, csrc/attention.cu) is here a fixed 256 KB array inside the library's device image, so the
+ * call performs no cudaMalloc / cudaFree / pool operation of any kind.  Limits and caveats:
+ *   - sequences x heads (sequences = windows in GLOBAL mode, windows*W in FRAME mode) must be <= 65536 on that path,
+ *     else MF_ERR_UNSUPPORTED (nothing enqueued); the other paths (head_dim 128, shorter sequences) use no scratch and
+ *     have no such limit;
+ *   - every call on a device shares the array (it is cleared by each call before use): calls that may overlap on the
+ *     GPU (different streams, concurrent graph launches) race on it -- serialise them or use mf_window_attention;
+ *   - the array is held by every GPU that loads the library, until the process exits.
+ */
+mf_status mf_window_attention_noalloc(const void* q, const void* k, const void* v, void* out, float* lse,
+                                      int windows, int frames_per_window, int tokens_per_frame, int heads,
+                                      int head_dim, mf_attn_mode mode, float softmax_scale, void* stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Host-buffer conveniences (end-to-end path): same semantics, every pointer is HOST memory
  * (pinned memory makes the copies asynchronous).  They allocate device buffers, copy in,

@@ -22,7 +22,7 @@ EXPORTS = ["mf_status_string", "mf_last_error", "mf_version", "mf_num_windows", 
            "mf_window_attention_host", "mf_chain_and_focus_host", "mf_linear", "mf_layernorm",
            "mf_block_workspace_size", "mf_block_forward", "mf_chain_state_size", "mf_chain_poses_step", "mf_motion_focus_upsampled",
            "mf_align_depth_workspace_size", "mf_align_depth",
-           "mf_align_depth_state_size", "mf_align_depth_step"]
+           "mf_align_depth_state_size", "mf_align_depth_step", "mf_window_attention_noalloc"]
 
 
 class MfError(RuntimeError):
@@ -62,6 +62,7 @@ def lib():
         L.mf_num_windows.argtypes = [ci, ci, ci]
         L.mf_window_start.argtypes = [ci, ci, ci, ci]
         L.mf_window_attention.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, cf, vp]
+        L.mf_window_attention_noalloc.argtypes = L.mf_window_attention.argtypes
         L.mf_chain_poses.argtypes = [vp, ci, ci, ci, ci, ci, ci, vp, vp]
         L.mf_motion_focus_workspace_size.restype = ctypes.c_size_t
         L.mf_motion_focus_workspace_size.argtypes = [ci, ci, ci, ci]
@@ -126,8 +127,10 @@ def window_starts(num_frames, w, stride):
 
 
 def window_attention(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLOBAL, softmax_scale=0.0,
-                     out=None, return_lse=False):
-    """q,k,v: bf16 CUDA [windows, S, H, D] with S = frames_per_window*tokens_per_frame."""
+                     out=None, return_lse=False, noalloc=False):
+    """q,k,v: bf16 CUDA [windows, S, H, D] with S = frames_per_window*tokens_per_frame.  noalloc=True calls
+    mf_window_attention_noalloc (static scratch inside the library, include/mf.h); pass `out` as well if this
+    binding must not create a tensor either."""
     for name, t in (("q", q), ("k", k), ("v", v)):
         _dev(t, torch.bfloat16, name)
     if q.dim() != 4 or k.shape != q.shape or v.shape != q.shape:
@@ -139,9 +142,9 @@ def window_attention(q, k, v, frames_per_window, tokens_per_frame, mode=ATTN_GLO
         out = torch.empty_like(q)
     _dev(out, torch.bfloat16, "out")
     lse = torch.empty((windows, heads, s_len), device=q.device, dtype=torch.float32) if return_lse else None
-    _check(lib().mf_window_attention(_ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse), windows,
-                                     frames_per_window, tokens_per_frame, heads, dim, mode,
-                                     float(softmax_scale), _stream()))
+    fn = lib().mf_window_attention_noalloc if noalloc else lib().mf_window_attention
+    _check(fn(_ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse), windows, frames_per_window, tokens_per_frame, heads, dim, mode,
+              float(softmax_scale), _stream()))
     return (out, lse) if return_lse else out
 
 

@@ -655,3 +655,102 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     if (bound_ws) MF_CUDA_OK(cudaFreeAsync(bound_ws, cs));
     return MF_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// mf_window_attention_noalloc: the same attention for callers that cannot allocate (include/mf.h)
+// ------------------------------------------------------------------------------------------------
+namespace mf {
+
+// The score bound's scratch ([sequences, heads] floats, see key_norm_max_kernel) as a fixed array in the library's own
+// device image instead of a stream-ordered allocation: 64 Ki entries = 256 KB, held by every GPU that loads the library
+// until the process exits.  In host code `g_bound_scratch` is only a stand-in for the symbol, not a device address: the
+// address comes from cudaGetSymbolAddress, once per device, with that device current (static_bound_scratch below).
+constexpr int kStaticBoundEntries = 65536;
+static __device__ __align__(256) uint32_t g_bound_scratch[kStaticBoundEntries];
+
+static mf_status static_bound_scratch(uint32_t** p) {
+    static std::atomic<uint32_t*> addr[64];
+    int dev = 0;
+    MF_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(MF_ERR_UNSUPPORTED, "device ordinal %d", dev);
+    uint32_t* a = addr[dev].load(std::memory_order_acquire);
+    if (!a) {
+        void* sym = nullptr;
+        MF_CUDA_OK(cudaGetSymbolAddress(&sym, g_bound_scratch));          // (this device's copy of the array)
+        if (!sym) return fail(MF_ERR_CUDA, "cudaGetSymbolAddress returned NULL");
+        a = static_cast<uint32_t*>(sym);
+        addr[dev].store(a, std::memory_order_release);
+    }
+    *p = a;
+    return MF_OK;
+}
+
+}  // namespace mf
+
+extern "C" mf_status mf_window_attention_noalloc(const void* q, const void* k, const void* v, void* out, float* lse,
+                                                 int windows, int frames_per_window, int tokens_per_frame, int heads,
+                                                 int head_dim, mf_attn_mode mode, float softmax_scale, void* stream) {
+    using namespace mf;
+    mf_status st;
+    {   // every argument check of mf_window_attention, nothing enqueued
+        const bool outer_dry_run = validate_only();
+        validate_only() = true;
+        st = mf_window_attention(q, k, v, out, lse, windows, frames_per_window, tokens_per_frame, heads, head_dim, mode,
+                                 softmax_scale, stream);
+        validate_only() = outer_dry_run;
+        if (st != MF_OK || outer_dry_run) return st;
+    }
+    const int sequences = mode == MF_ATTN_FRAME ? windows * frames_per_window : windows;
+    const int seq_len = mode == MF_ATTN_FRAME ? tokens_per_frame : frames_per_window * tokens_per_frame;
+    // head_dim 128 and the short sequences of the persistent kernel use no scratch memory: mf_window_attention allocates
+    // nothing on those paths and is the entry point for them as it stands
+    if (head_dim == 128 || ((seq_len + kBN - 1) / kBN < kPersistentBelowTiles && heads <= 65535 && sequences <= 65535))
+        return mf_window_attention(q, k, v, out, lse, windows, frames_per_window, tokens_per_frame, heads, head_dim, mode,
+                                   softmax_scale, stream);
+    // long sequences, head_dim 64: window_attention_kernel with the score bound in the static array
+    const long long entries = static_cast<long long>(sequences) * heads;
+    if (entries > kStaticBoundEntries || heads > 4096)
+        return fail(MF_ERR_UNSUPPORTED, "mf_window_attention_noalloc: sequences x heads = %lld exceeds the static scratch (%d entries); "
+                    "use mf_window_attention", entries, kStaticBoundEntries);
+    uint32_t* scratch = nullptr;
+    if ((st = static_bound_scratch(&scratch)) != MF_OK) return st;
+
+    AttnParams prm;
+    prm.seq_len = seq_len;
+    prm.heads = heads;
+    prm.q_blocks = (seq_len + kQTiles * kBM - 1) / (kQTiles * kBM);
+    const float scale = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf(static_cast<float>(head_dim));
+    prm.scale_log2 = scale * 1.4426950408889634f;
+    prm.out = static_cast<__nv_bfloat16*>(out);
+    prm.lse = lse;
+    prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
+    prm.key_norm2_max = reinterpret_cast<const float*>(scratch);
+    CUtensorMap mq, mk, mv;
+    if ((st = cached_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = cached_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;
+    if ((st = cached_map(&mv, v, sequences, seq_len, heads)) != MF_OK) return st;
+    const long long grid = static_cast<long long>(prm.q_blocks) * heads * sequences;
+    const int smem = static_cast<int>(sizeof(AttnSmem)) + 1024;
+    {   // (per-device kernel attribute, as in mf_window_attention)
+        static std::atomic<bool> attr_set[64];
+        int dev = 0;
+        MF_CUDA_OK(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
+            MF_CUDA_OK(cudaFuncSetAttribute(window_attention_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            if (dev >= 0 && dev < 64) attr_set[dev].store(true, std::memory_order_release);
+        }
+    }
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    // the array keeps the previous call's maxima: the entries this call uses start at zero again
+    MF_CUDA_OK(cudaMemsetAsync(scratch, 0, static_cast<size_t>(entries) * sizeof(uint32_t), cs));
+    const long long rows = static_cast<long long>(seq_len) * heads;
+    const long long want = (rows * 8 + 256 * 4 - 1) / (256 * 4);
+    const long long cap = (8LL * sm_count() + sequences - 1) / sequences;
+    const unsigned gx = static_cast<unsigned>(std::max(1LL, std::min(want, cap)));
+    key_norm_max_kernel<<<dim3(gx, static_cast<unsigned>(sequences)), 256, heads * sizeof(uint32_t), cs>>>(
+        static_cast<const uint4*>(k), scratch, rows, heads);
+    MF_CUDA_OK(cudaGetLastError());
+    window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, cs>>>(mq, mk, mv, prm);
+    MF_CUDA_OK(cudaGetLastError());
+    return MF_OK;
+}
