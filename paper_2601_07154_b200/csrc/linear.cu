@@ -88,10 +88,12 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
     constexpr int kBTile = Smem::kBTile;
     extern __shared__ uint8_t smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (warp number and cluster rank through a shuffle: warp-uniform to the compiler, so the role loops keep their addresses and
+    // descriptors in uniform registers and the single-lane TMA / MMA issue needs no per-instruction active-lane loop; attention.cu)
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
     const int n_tiles_total = prm.m_tiles * prm.n_tiles;
     const int k_steps = prm.K / kGK;
-    const int rank = kCtas == 2 ? static_cast<int>(ptx::cluster_ctarank()) : 0;     // 0 = leader of the pair
+    const int rank = kCtas == 2 ? __shfl_sync(0xffffffffu, static_cast<int>(ptx::cluster_ctarank()), 0) : 0;     // 0 = leader of the pair
     const int tile0 = blockIdx.x / kCtas, tile_step = gridDim.x / kCtas;
 
     if (warp == 0 && lane == 0) {
@@ -115,17 +117,19 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
     if (kCtas == 2) ptx::cluster_sync();
     else __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tmem = sm.tmem_base;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, sm.tmem_base, 0);
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
+        // ===================== TMA producer (whole warp in the loop, one elected lane issues) =====================
+        {
+            const bool leader = ptx::elect_one();
             int it = 0;
             for (int tile = tile0; tile < n_tiles_total; tile += tile_step) {
                 const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
                 for (int ks = 0; ks < k_steps; ++ks, ++it) {
                     const int st = it % kGStages;
                     ptx::mbar_wait(&sm.empty[st], ((it / kGStages) & 1) ^ 1);
+                    if (!leader) continue;
                     if (kCtas == 1) {
                         ptx::mbar_arrive_expect_tx(&sm.full[st], kATile + kBTile);
                         tma_load_2d(sm.a[st], &map_x, &sm.full[st], ks * kGK, mt * kGM);
@@ -141,10 +145,12 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                     }
                 }
             }
+            __syncwarp();
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0 && rank == 0) {
+        // ===================== MMA issuer (whole warp in the loop, one elected lane issues) =====================
+        if (rank == 0) {
+            const bool leader = ptx::elect_one();
             int it = 0, local = 0;
             for (int tile = tile0; tile < n_tiles_total; tile += tile_step, ++local) {
                 const int buf = local & 1;
@@ -155,6 +161,7 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                     const int st = it % kGStages;
                     ptx::mbar_wait(&sm.full[st], (it / kGStages) & 1);
                     ptx::tc_fence_after();
+                    if (!leader) continue;
                     const uint64_t ad = ptx::smem_desc_sw128(ptx::smem_u32(sm.a[st]));
                     const uint64_t bd = ptx::smem_desc_sw128(ptx::smem_u32(sm.b[st]));
 #pragma unroll
@@ -165,9 +172,12 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                     if (kCtas == 2) ptx::mma_commit_pair(&sm.empty[st], 3);        // frees the stage in both CTAs
                     else ptx::mma_commit(&sm.empty[st]);
                 }
-                if (kCtas == 2) ptx::mma_commit_pair(&sm.acc_full[buf], 3);
-                else ptx::mma_commit(&sm.acc_full[buf]);
+                if (leader) {
+                    if (kCtas == 2) ptx::mma_commit_pair(&sm.acc_full[buf], 3);
+                    else ptx::mma_commit(&sm.acc_full[buf]);
+                }
             }
+            __syncwarp();
         }
     } else {
         // ===================== epilogue warps =====================
