@@ -316,6 +316,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     }
                 }
                 const uint64_t neg_m2 = ptx::pack2(-m_used, -m_used);
+                const uint64_t magic_minus_m2 = ptx::pack2(12582912.0f - m_used, 12582912.0f - m_used);       // (bound path: m_used is an integer)
                 uint64_t scale_h = scale2;
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
@@ -323,9 +324,14 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                     for (int c = 2 * h; c < 2 * h + 2 && c < kChunks; ++c) {
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
-                            ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
                             constexpr int kPolyPairs = kBounded ? MF_POLY_PAIRS_BOUND : MF_POLY_PAIRS;
-                            if (((((i >> 1) & 15) * kPolyPairs) & 15) < kPolyPairs) {       // kPolyPairs of every 16 pairs, evenly spread
+                            const bool poly = ((((i >> 1) & 15) * kPolyPairs) & 15) < kPolyPairs;       // kPolyPairs of every 16 pairs, evenly spread
+                            if (poly && kBounded && !kMasked) {           // straight from the raw scores (attention_common.cuh)
+                                exp2_poly2_bounded(s[c][i], s[c][i + 1], scale_h, magic_minus_m2);
+                                continue;
+                            }
+                            ptx::ffma2(s[c][i], s[c][i + 1], scale_h, neg_m2);
+                            if (poly) {
                                 exp2_poly2(s[c][i], s[c][i + 1]);
                             } else {
                                 s[c][i] = __float_as_uint(ptx::ex2(__uint_as_float(s[c][i])));
@@ -391,7 +397,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
                 const float kk = prm.key_norm2_max[static_cast<size_t>(seq) * prm.heads + head];
                 const float bound = sqrtf(qq * kk) * fabsf(prm.scale_log2) * (1.0f + 0x1p-10f);       // (slack: fp32 rounding of the sums and of S)
                 bounded = __all_sync(0xffffffffu, bound <= kScoreBoundMax);
-                if (bounded) m_used = bound;
+                if (bounded) m_used = ceilf(bound);         // an integer (exp2_poly2_bounded), at most kScoreBoundMax
             }
             if (bounded) all_tiles(std::true_type{});
             else all_tiles(std::false_type{});

@@ -48,6 +48,30 @@ __device__ __forceinline__ void exp2_poly2(uint32_t& a0, uint32_t& a1) {
     a1 = p1 + (t1 << 23);
 }
 
+// The same from the RAW scores on the score-bound path (attention.cu), where the subtracted constant m is an INTEGER and
+// x = s * scale - m lies in [-64, 0]:  t = s * scale + (magic - m) holds n = round(x) in its low bits after one FFMA (magic - m
+// is exact),  q = (magic - m) - t = -(n + m) exactly,  f = s * scale + q in [-0.5, 0.5] by a second FFMA.  No clamp (x >= -64
+// keeps 2^n p normal) and no separate scaling: 6 packed instructions + 2 integer per pair instead of 9 + 2.
+__device__ __forceinline__ void exp2_poly2_bounded(uint32_t& a0, uint32_t& a1, uint64_t scale2, uint64_t magic_minus_m2) {
+    const uint64_t c3 = ptx::pack2(0.055171407759189606f, 0.055171407759189606f);
+    const uint64_t c2 = ptx::pack2(0.24261075258255005f, 0.24261075258255005f);
+    const uint64_t c1 = ptx::pack2(0.6932609677314758f, 0.6932609677314758f);
+    const uint64_t c0 = ptx::pack2(0.9999281167984009f, 0.9999281167984009f);
+    uint64_t s, t, q, f, p;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(s) : "r"(a0), "r"(a1));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(s), "l"(scale2), "l"(magic_minus_m2));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(q) : "l"(magic_minus_m2), "l"(t));             // -(n + m)
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(f) : "l"(s), "l"(scale2), "l"(q));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(c3), "l"(f), "l"(c2));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c1));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p) : "l"(p), "l"(f), "l"(c0));
+    uint32_t p0, p1, t0, t1;
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(p0), "=r"(p1) : "l"(p));
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(t0), "=r"(t1) : "l"(t));
+    a0 = p0 + (t0 << 23);
+    a1 = p1 + (t1 << 23);
+}
+
 // head_dim 64, short sequences: persistent kernel driven by cluster launch control (attention_clc.cu); the caller supplies the
 // tensor maps of q, k, v and out (box 64 x 1 x 128 x 1, SWIZZLE_128B)
 mf_status launch_attention_clc(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
