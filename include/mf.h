@@ -55,6 +55,15 @@ int mf_version(void);         /* major*10000 + minor*100 + patch */
  * scores (accurate to 2^-8 absolute: it is formed from the bf16-rounded weights the PV product
  * uses), or NULL.  head_dim must be 64 or 128 (else MF_ERR_UNSUPPORTED).  softmax_scale <= 0
  * selects 1/sqrt(head_dim).
+ *
+ * Device memory: at head_dim 64, sequences of 32 KV tiles and more (S >= 3969) first run a pass over k that
+ * writes max |k|^2 per (sequence, head) into [sequences, heads] floats of scratch (the score bound of
+ * csrc/attention.cu).  That scratch is allocated and freed ON `stream` from a memory pool owned by the
+ * library (cudaMallocFromPoolAsync / cudaFreeAsync: no synchronisation, legal under stream capture, safe
+ * with concurrent callers on other streams).  Every other path of this call allocates nothing.
+ * mf_window_attention_noalloc below is the same call with that scratch in a static device array.
+ * Rows whose bound |q_i| max_j|k_j| scale log2(e) exceeds 32, or holds NaN / Inf, take the exact
+ * online-softmax path; the result is within the same bars either way.
  */
 typedef enum { MF_ATTN_GLOBAL = 0, MF_ATTN_FRAME = 1 } mf_attn_mode;
 
