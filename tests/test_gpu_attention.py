@@ -163,6 +163,40 @@ def test_score_bound_far_above_the_scores(api):
     _compare(api, q2, k2, v2, s_len, _long_rows(s_len, 3))
 
 
+def _long_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    return [(int(rng.integers(1, 4)), int(rng.integers(1, 5)), int(rng.integers(4000, 9000)), int(rng.integers(1, 7)), int(rng.integers(0, 2)),
+             int(rng.integers(0, 1 << 30))) for _ in range(n)]
+
+
+@pytest.mark.parametrize("windows,w,s_target,heads,mode,seed", _long_cases(10, 20260110))
+def test_random_long_sequences_mixed_scales(api, windows, w, s_target, heads, mode, seed):
+    # Seeded random shapes on the one-item kernel (32 KV tiles and more per sequence, either mode), every block of 1..200 rows with
+    # its own query scale from {0.5, 1, 2, 4, 8}: warps on the score-bound path, on the exact path and mixed, ragged tails anywhere.
+    rng = np.random.default_rng(seed)
+    p = s_target if mode == oa.FRAME else max(1, s_target // w)
+    s_len = w * p
+    q, k, v = synth.qkv(windows, s_len, heads, 64, seed, device="cuda")
+    f = torch.ones(s_len, device="cuda")
+    i = 0
+    while i < s_len:
+        n = int(rng.integers(1, 200))
+        f[i:i + n] = float(rng.choice([0.5, 1.0, 2.0, 4.0, 8.0]))
+        i += n
+    q = (q.float() * f[None, :, None, None]).to(torch.bfloat16)
+    rows = np.unique(np.concatenate([np.arange(33), np.arange(s_len - 140, s_len), rng.integers(0, s_len, 60)]))
+    out, lse = api.window_attention(q, k, v, w, p, mode, return_lse=True)
+    torch.cuda.synchronize()
+    ref, lse_ref = oa.window_attention(_to64(q), _to64(k), _to64(v), w, p, mode, rows=rows)
+    got = _to64(out)[:, rows]
+    assert np.isfinite(_to64(out)).all()
+    for n in range(windows):
+        d = got[n] - ref[n]
+        assert np.abs(d).max() <= MAX_ABS and np.linalg.norm(d) / np.linalg.norm(ref[n]) <= REL_L2
+        _per_row(d, ref[n], (windows, w, p, heads, mode, n))
+    assert np.abs(lse.cpu().numpy().astype(np.float64)[:, :, rows] - lse_ref).max() <= 4e-3
+
+
 def test_persistent_kernel_many_items_per_cta(api):
     # 148 SMs, 6000 work items of 2 KV tiles each: every CTA of the persistent kernel takes ~40 items through cluster launch
     # control; items with a dead second Q tile (S = 200 < 256... every item here) and live ones (S = 300) interleave per sequence
