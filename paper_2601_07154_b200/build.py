@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libmf_b200.so")
-SOURCES = ["api.cu", "api_host.cu", "chain.cu", "focus.cu", "attention.cu", "linear.cu", "depth.cu", "attention_d128.cu", "attention_clc.cu"]
+SOURCES = ["api.cu", "api_host.cu", "chain.cu", "focus.cu", "attention.cu", "linear.cu", "depth.cu", "attention_d128.cu", "attention_clc.cu", "attention_split.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 # chain.cu / focus.cu hold the bit-exact fp64 path: never contract mul+add into FMA there.

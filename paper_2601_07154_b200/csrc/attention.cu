@@ -48,7 +48,7 @@ constexpr int kPH = 32;                // TMEM columns of one P half (64 keys, b
 constexpr float kRescaleThreshold = 8.0f;
 constexpr float kScoreBoundMax = 32.0f;    // log2 units: the score-bound path is taken for rows with |q| max|k| scale log2(e) <= 32 (22 nats)
 #ifndef MF_POLY_PAIRS_BOUND
-#define MF_POLY_PAIRS_BOUND 6          // the same on the score-bound path, which has issue slots to spare (5: -0.6 %, 7: -2.3 %)
+#define MF_POLY_PAIRS_BOUND 7          // the same on the score-bound path (attention_split.cu: 4 .. 8 of 16 give 989 / 998 / 1014 / 1021 / 1022 TFLOP/s; this kernel alone: best at 6)
 #endif
 #ifndef MF_PERSISTENT_BELOW_TILES
 #define MF_PERSISTENT_BELOW_TILES 32   // sequences of fewer KV tiles (S <= 3968) run on the persistent kernel (attention_clc.cu); with the score-bound path here, S = 6216 gains 4 % on this kernel, S = 1024 loses 19 %
@@ -99,6 +99,7 @@ window_attention_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_
     // per-instruction loop over "active lanes" (measured on the campus launch: MMA issuers +1.3 %, producer +1.0 %, softmax
     // warps +2.2 %).
     const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+    if (prm.only_flagged != nullptr && prm.only_flagged[blockIdx.x] == 0u) return;      // done by window_attention_split_kernel
 
     // work item: q block fastest so that concurrently running CTAs share one head's K/V in L2
     const int qb = blockIdx.x % prm.q_blocks;
@@ -616,6 +617,7 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
     prm.lse = lse;
     prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
     prm.key_norm2_max = nullptr;
+    prm.only_flagged = nullptr;
     if (head_dim == 128)       // re-tiled variant (attention_d128.cu); q_blocks is the same: 256 query rows per CTA
         return launch_attention_d128(q, k, v, sequences, seq_len, heads, prm, static_cast<cudaStream_t>(stream));
 
@@ -643,7 +645,9 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
 #ifndef MF_NO_SCORE_BOUND          // (test builds: tests/test_gpu_attention_differential.py compares the exact paths of the two kernels bit for bit)
     if (heads <= 4096 && sequences <= 65535) {
         // the score bound's pass over K (window_attention_kernel: "Score bound"); 0.3 % of the attention launch at S = 24864
-        const size_t ws_bytes = static_cast<size_t>(sequences) * heads * sizeof(uint32_t);
+        // scratch: [sequences, heads] key norms, then one flag per CTA of the attention grid (attention_split.cu)
+        const size_t norm_words = static_cast<size_t>(sequences) * heads;
+        const size_t ws_bytes = (norm_words + static_cast<size_t>(grid)) * sizeof(uint32_t);
         if ((st = bound_workspace(&bound_ws, ws_bytes, cs)) != MF_OK) return st;
         MF_CUDA_OK(cudaMemsetAsync(bound_ws, 0, ws_bytes, cs));
         const long long rows = static_cast<long long>(seq_len) * heads;
@@ -654,6 +658,12 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
             static_cast<const uint4*>(k), bound_ws, rows, heads);
         MF_CUDA_OK(cudaGetLastError());
         prm.key_norm2_max = reinterpret_cast<const float*>(bound_ws);
+#ifndef MF_NO_SPLIT
+        // CTAs whose rows are all within the bound: four softmax warps per scheduler (attention_split.cu); the others are flagged
+        // there and done by the launch below, which returns at once from the rest
+        if ((st = launch_attention_split(mq, mk, mv, grid, prm, bound_ws + norm_words, cs)) != MF_OK) return st;
+        prm.only_flagged = bound_ws + norm_words;
+#endif
     }
 #endif
     window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, cs>>>(mq, mk, mv, prm);
@@ -731,6 +741,7 @@ extern "C" mf_status mf_window_attention_noalloc(const void* q, const void* k, c
     prm.lse = lse;
     prm.lse_frames = mode == MF_ATTN_FRAME ? frames_per_window : 1;
     prm.key_norm2_max = reinterpret_cast<const float*>(scratch);
+    prm.only_flagged = nullptr;
     CUtensorMap mq, mk, mv;
     if ((st = cached_map(&mq, q, sequences, seq_len, heads)) != MF_OK) return st;
     if ((st = cached_map(&mk, k, sequences, seq_len, heads)) != MF_OK) return st;

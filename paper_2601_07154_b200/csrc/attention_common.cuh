@@ -22,6 +22,7 @@ struct AttnParams {
     float* lse;         // [windows, heads, S] or nullptr
     int lse_frames;     // sequences per window (W in frame mode, 1 in global mode)
     const float* key_norm2_max;   // [sequences, heads] max over the keys of |k|^2 (attention.cu: the score bound), or nullptr
+    const uint32_t* only_flagged; // window_attention_kernel: if not nullptr, CTAs whose word is 0 return at once (attention_split.cu did them)
 };
 
 // (2^x0, 2^x1) on the FMA pipe.  x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a cubic (minimax in
@@ -76,6 +77,11 @@ __device__ __forceinline__ void exp2_poly2_bounded(uint32_t& a0, uint32_t& a1, u
 // tensor maps of q, k, v and out (box 64 x 1 x 128 x 1, SWIZZLE_128B)
 mf_status launch_attention_clc(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
                                int sequences, int seq_len, int heads, const AttnParams& prm, cudaStream_t stream);
+
+// head_dim 64, long sequences, CTAs whose rows are all within the score bound (attention_split.cu); the others set their word
+// of exact_flags (zeroed by the caller) and are left to window_attention_kernel
+mf_status launch_attention_split(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, long long grid,
+                                 const AttnParams& prm, uint32_t* exact_flags, cudaStream_t stream);
 
 // head_dim 128 variant (attention_d128.cu); same contract as the head_dim 64 launch inside mf_window_attention
 mf_status launch_attention_d128(const void* q, const void* k, const void* v, int sequences, int seq_len, int heads,

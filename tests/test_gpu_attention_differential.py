@@ -67,3 +67,41 @@ def test_persistent_kernel_short_items(libs, s_len, seqs, heads):
     a, la = _run(new, q, k, v, seqs, 1, s_len, heads, 0)
     b, lb = _run(old, q, k, v, seqs, 1, s_len, heads, 0)
     assert torch.equal(a, b) and torch.equal(la, lb)
+
+
+@pytest.fixture(scope="module")
+def nosplit(tmp_path_factory):
+    from paper_2601_07154_b200 import api, build
+    tmp = tmp_path_factory.mktemp("nosplit")
+    other = build.build(out=str(tmp / "libmf_nosplit.so"), extra_flags=["-DMF_NO_SPLIT"], build_dir=str(tmp / "obj"))
+    new = api.lib()
+    old = ctypes.CDLL(other)
+    old.mf_window_attention.argtypes = new.mf_window_attention.argtypes
+    return new, old
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_split_kernel_equals_one_item_kernel_bit_for_bit(nosplit, seed):
+    # Long sequences: CTAs whose rows are all within the score bound run on attention_split.cu (each row's 128 scores per KV
+    # tile split between two threads), the rest on attention.cu.  A build without the split kernel (-DMF_NO_SPLIT) runs every CTA
+    # on attention.cu, where such rows take the same score-bound arithmetic in one thread: outputs and lse must be bit-identical.
+    # Random shapes (ragged tails of every chunk count, dead second Q tiles), blocks of rows with larger query scales so that
+    # launches mix both kinds of CTA.
+    new, old = nosplit
+    rng = np.random.default_rng(seed)
+    for _ in range(12):
+        w, heads, windows, mode = int(rng.integers(1, 4)), int(rng.integers(1, 6)), int(rng.integers(1, 4)), int(rng.integers(0, 2))
+        s_target = int(rng.integers(3969, 9000))
+        p = s_target if mode == 1 else max(1, s_target // w)
+        s_len = w * p
+        q, k, v = synth.qkv(windows, s_len, heads, 64, int(rng.integers(0, 1 << 30)), device="cuda")
+        f = torch.ones(s_len, device="cuda")
+        for _ in range(int(rng.integers(0, 4))):
+            i = int(rng.integers(0, s_len))
+            f[i:i + int(rng.integers(1, 600))] = 8.0
+        q = (q.float() * f[None, :, None, None]).to(torch.bfloat16)
+        case = dict(windows=windows, w=w, p=p, heads=heads, mode=mode)
+        a, la = _run(new, q, k, v, windows, w, p, heads, mode)
+        b, lb = _run(old, q, k, v, windows, w, p, heads, mode)
+        assert torch.isfinite(a.float()).all(), case
+        assert torch.equal(a, b) and torch.equal(la, lb), case
