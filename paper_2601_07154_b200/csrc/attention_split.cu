@@ -129,6 +129,13 @@ window_attention_split_kernel(const __grid_constant__ CUtensorMap map_q, const _
         ptx::mbar_arrive_expect_tx(a_q_full, (tile1_live ? 2 : 1) * kTileBytes);
         ptx::tma_load_4d(sb + offsetof(Smem, q), &map_q, a_q_full, 0, head, row0, seq);
         if (tile1_live) ptx::tma_load_4d(sb + offsetof(Smem, q) + kTileBytes, &map_q, a_q_full, 0, head, row0 + kBM, seq);
+        // the first K/V stages go out before the decision (no wait needed: the ring is empty), so that it costs no load latency
+        for (int j = 0; j < kStages && j < n_kv; ++j) {
+            ptx::mbar_arrive_expect_tx(sb + offsetof(Smem, k_full) + 8 * j, kTileBytes);
+            ptx::tma_load_4d(sb + offsetof(Smem, k) + kTileBytes * j, &map_k, sb + offsetof(Smem, k_full) + 8 * j, 0, head, j * kBN, seq);
+            ptx::mbar_arrive_expect_tx(sb + offsetof(Smem, v_full) + 8 * j, kTileBytes);
+            ptx::tma_load_4d(sb + offsetof(Smem, v) + kTileBytes * j, &map_v, sb + offsetof(Smem, v_full) + 8 * j, 0, head, j * kBN, seq);
+        }
     }
     __syncwarp();
     const int tile = (warp >> 2) & 1, half = (warp >> 3) & 1;            // (softmax warps)
@@ -155,9 +162,14 @@ window_attention_split_kernel(const __grid_constant__ CUtensorMap map_q, const _
         m_used = ceilf(bound);
     }
     if (__syncthreads_or(outside)) {
-        // window_attention_kernel does this CTA.  (The Q loads have landed: every live softmax thread waited for them; a CTA
-        // with a dead second tile loaded only the first.)
+        // window_attention_kernel does this CTA.  Shared memory must outlive the loads in flight: the Q loads have landed (every
+        // live softmax thread waited for them); the K/V stages sent ahead are waited for here.
         if (threadIdx.x == 0) exact_flags[blockIdx.x] = 1u;
+        if (warp == 16)
+            for (int j = 0; j < kStages && j < n_kv; ++j) {
+                ptx::mbar_wait(sb + offsetof(Smem, k_full) + 8 * j, 0);
+                ptx::mbar_wait(sb + offsetof(Smem, v_full) + 8 * j, 0);
+            }
         ptx::tc_fence_before();
         __syncthreads();
         if (warp == 17) ptx::tmem_dealloc(tmem, kTmemCols);
@@ -172,7 +184,7 @@ window_attention_split_kernel(const __grid_constant__ CUtensorMap map_q, const _
         if (warp == 16) {
             // ===================== TMA producer (whole warp in the loop, one elected lane issues) =====================
             const bool leader = ptx::elect_one();
-            for (int j = 0; j < n_kv; ++j) {
+            for (int j = kStages; j < n_kv; ++j) {           // (stages 0 .. kStages-1 were sent before the decision)
                 const int st = j % kStages;
                 const uint32_t ph = (j / kStages) & 1;
                 ptx::mbar_wait(sb + offsetof(Smem, k_empty) + 8 * st, ph ^ 1);
