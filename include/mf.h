@@ -216,7 +216,9 @@ mf_status mf_motion_focus_upsampled(const double* global_w2c, mf_intrinsics K, i
  * call performs no cudaMalloc / cudaFree / pool operation of any kind.  Limits and caveats:
  *   - sequences x heads (sequences = windows in GLOBAL mode, windows*W in FRAME mode) must be <= 65536 on that path,
  *     else MF_ERR_UNSUPPORTED (nothing enqueued); the other paths (head_dim 128, shorter sequences) use no scratch and
- *     have no such limit;
+ *     have no such limit.  (Where sequences x heads + ceil(S/256) x heads x sequences also fits in 65536 words, the array
+ *     holds the per-CTA flags of csrc/attention_split.cu as well and the call runs the same kernels as
+ *     mf_window_attention; beyond that it runs window_attention_kernel alone: same results, ~4 % slower.);
  *   - every call on a device shares the array (it is cleared by each call before use): calls that may overlap on the
  *     GPU (different streams, concurrent graph launches) race on it -- serialise them or use mf_window_attention;
  *   - the array is held by every GPU that loads the library, until the process exits.

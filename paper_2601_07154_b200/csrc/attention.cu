@@ -767,6 +767,15 @@ extern "C" mf_status mf_window_attention_noalloc(const void* q, const void* k, c
     key_norm_max_kernel<<<dim3(gx, static_cast<unsigned>(sequences)), 256, heads * sizeof(uint32_t), cs>>>(
         static_cast<const uint4*>(k), scratch, rows, heads);
     MF_CUDA_OK(cudaGetLastError());
+#ifndef MF_NO_SPLIT
+    // where the array also holds one flag per CTA behind the norms, the score-bound CTAs run on attention_split.cu as in
+    // mf_window_attention (same results bit for bit either way)
+    if (entries + grid <= kStaticBoundEntries) {
+        MF_CUDA_OK(cudaMemsetAsync(scratch + entries, 0, static_cast<size_t>(grid) * sizeof(uint32_t), cs));
+        if ((st = launch_attention_split(mq, mk, mv, grid, prm, scratch + entries, cs)) != MF_OK) return st;
+        prm.only_flagged = scratch + entries;
+    }
+#endif
     window_attention_kernel<<<static_cast<unsigned>(grid), kThreads, smem, cs>>>(mq, mk, mv, prm);
     MF_CUDA_OK(cudaGetLastError());
     return MF_OK;
