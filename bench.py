@@ -158,8 +158,9 @@ class Workload:
     @staticmethod
     def attention_kernels(seq_len, head_dim):
         """Kernels of one mf_window_attention call: head_dim 64 sequences of 32 KV tiles and more run the key-norm pass of the
-        score bound (key_norm_max_kernel) ahead of window_attention_kernel (csrc/attention.cu)."""
-        return 2 if head_dim == 64 and (seq_len + 127) // 128 >= 32 else 1
+        score bound (key_norm_max_kernel), window_attention_split_kernel (the CTAs within the bound) and window_attention_kernel
+        (the others; csrc/attention.cu, attention_split.cu)."""
+        return 3 if head_dim == 64 and (seq_len + 127) // 128 >= 32 else 1
 
     @staticmethod
     def flops_per_step(cfg_idx, args, api):
@@ -746,8 +747,9 @@ def main():
     value = replicas.whole_job_value(wl.N, ms_step, world)
     tflops, focus_gbs = res["tflops"], res["focus_gbs"]
     traffic = ncu_traffic(args.config, wl.B)
-    roofline = {"bound": "tensor", "kernel": "window_attention_kernel (GLOBAL mode; the time is the whole mf_window_attention call: key_norm_max_kernel, "
-                                                   "the pass over K for the score bound, runs ahead of it on the same stream)", "achieved": tflops,
+    roofline = {"bound": "tensor", "kernel": "window_attention_split_kernel (GLOBAL mode; the time is the whole mf_window_attention call: "
+                                                   "key_norm_max_kernel, the pass over K for the score bound, runs ahead of it and window_attention_kernel, "
+                                                   "for CTAs outside the bound, behind it on the same stream)", "achieved": tflops,
                 "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": tflops / peaks["tf_sustained"],
                 "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['source']}); kernel timed inside a long step",
                 "frac_of_burst": tflops / peaks["tf_burst"], "frac_of_nominal_2250": tflops / 2250.0,
