@@ -647,7 +647,8 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
         // the score bound's pass over K (window_attention_kernel: "Score bound"); 0.3 % of the attention launch at S = 24864
         // scratch: [sequences, heads] key norms, then one flag per CTA of the attention grid (attention_split.cu)
         const size_t norm_words = static_cast<size_t>(sequences) * heads;
-        const size_t ws_bytes = (norm_words + static_cast<size_t>(grid)) * sizeof(uint32_t);
+        const bool split = grid <= (1LL << 24);          // (64 MB of flags at most; larger grids run window_attention_kernel alone)
+        const size_t ws_bytes = (norm_words + (split ? static_cast<size_t>(grid) : 0)) * sizeof(uint32_t);
         if ((st = bound_workspace(&bound_ws, ws_bytes, cs)) != MF_OK) return st;
         MF_CUDA_OK(cudaMemsetAsync(bound_ws, 0, ws_bytes, cs));
         const long long rows = static_cast<long long>(seq_len) * heads;
@@ -661,8 +662,12 @@ extern "C" mf_status mf_window_attention(const void* q, const void* k, const voi
 #ifndef MF_NO_SPLIT
         // CTAs whose rows are all within the bound: four softmax warps per scheduler (attention_split.cu); the others are flagged
         // there and done by the launch below, which returns at once from the rest
-        if ((st = launch_attention_split(mq, mk, mv, grid, prm, bound_ws + norm_words, cs)) != MF_OK) return st;
-        prm.only_flagged = bound_ws + norm_words;
+        if (split) {
+            if ((st = launch_attention_split(mq, mk, mv, grid, prm, bound_ws + norm_words, cs)) != MF_OK) return st;
+            prm.only_flagged = bound_ws + norm_words;
+        }
+#else
+        (void)split;
 #endif
     }
 #endif
