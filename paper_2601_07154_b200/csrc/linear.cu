@@ -27,7 +27,10 @@ namespace mf {
 
 constexpr int kGM = 128, kGN = 256, kGK = 64;
 constexpr int kEpiWarps = 8;               // two per TMEM lane quarter: each takes half of the tile's 256 columns
-constexpr int kGThreads = (2 + kEpiWarps) * 32;
+constexpr int kGThreads = (4 + kEpiWarps) * 32;   // warpgroup 0: TMA producer, MMA issuer and two idle warps; warpgroups 1-2: the epilogue warps
+// (A CTA of 10 warps is allocated as 12 anyway, which capped the kernel at 168 registers per thread and made ptxas spill the
+// epilogue's residual prefetch: the spill store then waited for the loads in front of every tile.  With 12 warps setmaxnreg
+// moves warpgroup 0's registers to the epilogue warps: 56 / 224.)
 constexpr int kATile = kGM * kGK * 2;      // 16 KB
 
 // kCtas = 1: one CTA per 128 x 256 output tile.  kCtas = 2: a CTA pair (cluster of 2, tcgen05 cta_group::2) per 256 x 256
@@ -119,6 +122,8 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
     ptx::tc_fence_after();
     const uint32_t tmem = __shfl_sync(0xffffffffu, sm.tmem_base, 0);
 
+    if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     if (warp == 0) {
         // ===================== TMA producer (whole warp in the loop, one elected lane issues) =====================
         {
@@ -179,16 +184,18 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
             }
             __syncwarp();
         }
+    }
     } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== epilogue warps =====================
         // A thread owns one output row (TMEM lane) and 64 consecutive columns per pass.  Rows are 2-8 KB apart in
         // global memory, so the 32 x 128 B block of a pass goes through a per-warp, XOR-swizzled staging buffer: global
         // accesses are then 4 rows x 128 B per warp instruction (4 wavefronts instead of 32), for the stores and for
         // the residual loads alike.
         const int quarter = warp & 3;                      // TMEM lanes 32*quarter .. +31
-        const int chalf = (warp - 2) >> 2;                 // columns [128*chalf, 128*chalf + 128) of the tile
+        const int chalf = (warp - 4) >> 2;                 // columns [128*chalf, 128*chalf + 128) of the tile
         const uint32_t lane_addr = static_cast<uint32_t>(quarter * 32) << 16;
-        uint4* stage = reinterpret_cast<uint4*>(sm.stage[warp - 2]);      // [32 rows][8 chunks of 16 B]
+        uint4* stage = reinterpret_cast<uint4*>(sm.stage[warp - 4]);      // [32 rows][8 chunks of 16 B]
         const int crow = lane >> 3, cchunk = lane & 7;     // coalesced phase: this lane's row (of 4) and 16-byte chunk
         int local = 0;
         for (int tile = tile0; tile < n_tiles_total; tile += tile_step, ++local) {
