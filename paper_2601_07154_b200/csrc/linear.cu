@@ -77,6 +77,40 @@ __device__ __forceinline__ float gelu_erf(float v) {
     return 0.5f * v * (1.0f + copysignf(erf_abs, v));
 }
 
+// The same for two values with packed f32x2 instructions (the same operations in the same order per element, so the result is
+// the scalar form's bit for bit): 13 packed + 4 logic + 4 MUFU instructions per pair instead of 32 + 4.
+__device__ __forceinline__ void gelu_erf2(float& v0, float& v1) {
+    const uint64_t v = ptx::pack2(v0, v1);
+    const uint64_t ax = ptx::pack2(fabsf(v0), fabsf(v1));
+    uint64_t x, d, poly, arg, pt, ea, r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(x) : "l"(ax), "l"(ptx::pack2(0.70710678118654752f, 0.70710678118654752f)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(ptx::pack2(0.3275911f, 0.3275911f)), "l"(x), "l"(ptx::pack2(1.0f, 1.0f)));
+    float d0, d1, t0, t1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(d));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t0) : "f"(d0));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t1) : "f"(d1));
+    const uint64_t t = ptx::pack2(t0, t1);
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(poly) : "l"(ptx::pack2(1.061405429f, 1.061405429f)), "l"(t), "l"(ptx::pack2(-1.453152027f, -1.453152027f)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(poly) : "l"(poly), "l"(t), "l"(ptx::pack2(1.421413741f, 1.421413741f)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(poly) : "l"(poly), "l"(t), "l"(ptx::pack2(-0.284496736f, -0.284496736f)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(poly) : "l"(poly), "l"(t), "l"(ptx::pack2(0.254829592f, 0.254829592f)));
+    // (-x * x) * log2(e), then e = 2^that
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(arg) : "l"(x ^ 0x8000000080000000ull), "l"(x));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(arg) : "l"(arg), "l"(ptx::pack2(1.4426950408889634f, 1.4426950408889634f)));
+    float a0, a1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(arg));
+    const uint64_t e = ptx::pack2(ptx::ex2(a0), ptx::ex2(a1));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(pt) : "l"(poly ^ 0x8000000080000000ull), "l"(t));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ea) : "l"(pt), "l"(e), "l"(ptx::pack2(1.0f, 1.0f)));
+    // copysign(erf_abs, v); 0.5 v (1 + that)
+    const uint64_t cs = (ea & 0x7fffffff7fffffffull) | (v & 0x8000000080000000ull);
+    uint64_t one_cs, hv;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(one_cs) : "l"(ptx::pack2(1.0f, 1.0f)), "l"(cs));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(hv) : "l"(ptx::pack2(0.5f, 0.5f)), "l"(v));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(hv), "l"(one_cs));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(v0), "=f"(v1) : "l"(r));
+}
+
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
                  :: "r"(ptx::smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(ptx::smem_u32(bar)), "r"(c0), "r"(c1)
@@ -257,7 +291,7 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                     }
                     if (prm.act == MF_ACT_GELU) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) vals[i] = gelu_erf(vals[i]);
+                        for (int i = 0; i < 8; i += 2) gelu_erf2(vals[i], vals[i + 1]);
                     }
                     if (prm.residual) {
                         const uint32_t rr[4] = {myres[j].x, myres[j].y, myres[j].z, myres[j].w};
