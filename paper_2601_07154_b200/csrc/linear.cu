@@ -232,6 +232,21 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
         uint4* stage = reinterpret_cast<uint4*>(sm.stage[warp - 4]);      // [32 rows][8 chunks of 16 B]
         const int crow = lane >> 3, cchunk = lane & 7;     // coalesced phase: this lane's row (of 4) and 16-byte chunk
         int local = 0;
+        // Residual: the 32 x 128 B block of ONE pass is in flight in registers at a time (coalesced loads), issued a whole pass
+        // ahead: pass 1's while pass 0 is computed, the next tile's pass 0 while pass 1 is.
+        uint4 rres[8];
+        auto load_residual = [&](int t, int g) {
+            const int t_mt = t / prm.n_tiles, t_nt = t - t_mt * prm.n_tiles;
+            const int t_row0 = t_mt * (kCtas * kGM) + rank * kGM + quarter * 32;
+            const int t_n0 = t_nt * kGN + 128 * chalf;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int r = t_row0 + 4 * i + crow;
+                rres[i] = r < prm.M ? __ldg(reinterpret_cast<const uint4*>(prm.residual + static_cast<size_t>(r) * prm.N + t_n0 + 64 * g + 8 * cchunk))
+                                    : make_uint4(0u, 0u, 0u, 0u);
+            }
+        };
+        if (prm.residual && tile0 < n_tiles_total) load_residual(tile0, 0);
         for (int tile = tile0; tile < n_tiles_total; tile += tile_step, ++local) {
             const int buf = local & 1;
             const int mt = tile / prm.n_tiles, nt = tile - mt * prm.n_tiles;
@@ -239,19 +254,6 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
             const int n0 = nt * kGN + 128 * chalf;         // first of this warp's 128 columns
             const int which = n0 / prm.n_split, c0 = n0 - which * prm.n_split;
             __nv_bfloat16* dst = prm.out[which] + c0;
-            // residual of both passes, fetched (coalesced) before the accumulator is waited for
-            uint4 rres[2][8];
-            if (prm.residual) {
-#pragma unroll
-                for (int g = 0; g < 2; ++g)
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int r = row0 + 4 * i + crow;
-                        rres[g][i] = r < prm.M ? __ldg(reinterpret_cast<const uint4*>(prm.residual + static_cast<size_t>(r) * prm.N +
-                                                                                      n0 + 64 * g + 8 * cchunk))
-                                               : make_uint4(0u, 0u, 0u, 0u);
-                    }
-            }
             ptx::mbar_wait(&sm.acc_full[buf], (local >> 1) & 1);
             ptx::tc_fence_after();
 #pragma unroll
@@ -263,11 +265,13 @@ linear_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_constant__
                 if (prm.residual) {
                     __syncwarp();
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) stage[(4 * i + crow) * 8 + (cchunk ^ ((4 * i + crow) & 7))] = rres[g][i];
+                    for (int i = 0; i < 8; ++i) stage[(4 * i + crow) * 8 + (cchunk ^ ((4 * i + crow) & 7))] = rres[i];
                     __syncwarp();
 #pragma unroll
                     for (int j = 0; j < 8; ++j) myres[j] = stage[lane * 8 + (j ^ (lane & 7))];
                     __syncwarp();
+                    if (g == 0) load_residual(tile, 1);
+                    else if (tile + tile_step < n_tiles_total) load_residual(tile + tile_step, 0);
                 }
                 ptx::tc_wait_ld();
                 if (g == 1) {                              // the accumulator is in registers: hand it back to the MMA issuer
