@@ -19,6 +19,10 @@
 // Online softmax in fp32 with lazy rescaling (O and l are rescaled only when the running maximum grew by more
 // than 2^8); O is normalised by 1/l in the epilogue.  FRAME mode is GLOBAL mode on the same bytes viewed as
 // [windows*W, P, H, D].
+// Long sequences (32 KV tiles and more) first get max |k|^2 per (sequence, head) from key_norm_max_kernel; warps whose rows'
+// Cauchy-Schwarz score bound is small subtract that bound instead of a running maximum ("Score bound" in the softmax code), and
+// CTAs in which EVERY row is so bounded are done by window_attention_split_kernel (attention_split.cu: four softmax warps per
+// scheduler), this kernel taking only the CTAs flagged by it (AttnParams::only_flagged).  Shorter sequences: attention_clc.cu.
 #include "common.h"
 #include "sm100_ptx.cuh"
 #include "tensormap.h"
