@@ -70,7 +70,7 @@ const char* mf_status_string(mf_status s) {
 
 const char* mf_last_error(void) { return mf::error_buffer(); }
 
-int mf_version(void) { return 100; }
+int mf_version(void) { return 200; }     // 0.2.0: round 2 (mf_window_attention_noalloc, score-bound path)
 
 // P:70; tail window starts at num_frames - W (reading B6 in DESIGN.md).
 int mf_num_windows(int num_frames, int W, int stride) {
