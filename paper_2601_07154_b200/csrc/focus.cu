@@ -834,9 +834,11 @@ static mf_status motion_focus_impl(const double* global_w2c, mf_intrinsics K, in
 
     const int tc = (width + kTile - 1) / kTile, tr = (height + kTile - 1) / kTile;
     const size_t smem = sizeof(float) * (npad * static_cast<size_t>(tc + tr) + kMaxPoints + 8 * kTile * npad);
-    // CTAs per frame in norm_kernel: kNormBlocks when the call is short, fewer when it holds so many frames that 8 per frame
-    // would need several waves of these latency-bound CTAs (8 x 256 threads fit one SM)
-    const int norm_blocks = std::max(1, std::min(kNormBlocks, (8 * sm_count() + count - 1) / count));
+    // CTAs per frame in norm_kernel: kNormBlocks when the call is short, fewer when it holds so many frames that the call's CTAs
+    // would need several waves of these latency-bound CTAs: two of them (256 threads, 118 registers) are resident per SM.
+    // (Measured, 20 back-to-back calls: 1 / 2 / 3 / 4 / 8 / 16 CTAs per SM as the budget give 5451 / 5392 / 5384 / 5335 / 5180 /
+    // 5008 GB/s for 240 frames of 960x544 and 8626 / 8709 / 8663 / 8687 / 8685 / 8689 for 64 frames of 4K.)
+    const int norm_blocks = std::max(1, std::min(kNormBlocks, (2 * sm_count() + count - 1) / count));
     if (focus_map && smem > 200 * 1024) return fail(MF_ERR_UNSUPPORTED, "mf_motion_focus: image too large for the bound tables");
     if (validate_only()) return MF_OK;
     if (focus_map) {
